@@ -1,0 +1,241 @@
+"""ctypes/numpy face of the CPU oracle.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It never imports paper_1212_0785_b200 and shares no code with it.
+
+Fields are numpy arrays in the canonical lexicographic layout of oracle/qcd_oracle.h:
+    matrix field  complex128[V, 4, 3, 3]      real field  float64[V, ncomp]
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+ALL, EVEN, ODD = 0, 1, 2
+SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
+MAP_CB_OF_LEX, MAP_LEX_OF_CB, MAP_NBR_FWD0, MAP_NBR_BWD0, MAP_PARITY, MAP_TSLICE = 0, 1, 2, 6, 10, 11
+
+_c_int4 = C.c_int * 4
+_dp = C.POINTER(C.c_double)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _mat(a, V):
+    assert a.dtype == np.complex128 and a.flags.c_contiguous and a.shape == (V, 4, 3, 3), (a.dtype, a.shape)
+    return _ptr(a)
+
+
+class Oracle:
+    """One loaded oracle library (serial by default; omp=True loads the OpenMP build)."""
+
+    def __init__(self, omp=False):
+        serial, par = _build.build()
+        self.lib = C.CDLL(par if omp else serial)
+        self.omp = omp
+        L = self.lib
+        L.orc_rng_block.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
+                                    C.POINTER(C.c_uint32), _dp, _dp]
+        L.orc_rng_block.restype = None
+        L.orc_mom_refresh.argtypes = [_c_int4, C.c_int, C.c_uint64, C.c_uint32, _dp]
+        L.orc_hot_start.argtypes = [_c_int4, C.c_uint64, C.c_double, _dp]
+        L.orc_perturb.argtypes = [_c_int4, C.c_uint64, C.c_double, _dp]
+        L.orc_gauge_transform.argtypes = [_c_int4, C.c_uint64, C.c_double, _dp, _dp, _dp]
+        L.orc_plaquette.argtypes = [_c_int4, _dp, _dp, _dp]
+        L.orc_action.argtypes = [_c_int4, C.c_double, _dp, _dp]
+        L.orc_gauge_force.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp]
+        L.orc_sum_retr_w.argtypes = [_c_int4, _dp, _dp]
+        L.orc_mom_update.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp]
+        L.orc_link_update.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp, C.c_int]
+        L.orc_reunit.argtypes = [_c_int4, C.c_int, _dp]
+        L.orc_sum.argtypes = [_c_int4, C.c_int, C.c_int, C.c_int, _dp, _dp]
+        L.orc_sum_multi.argtypes = [_c_int4, C.c_int, C.c_int, _dp, C.POINTER(C.c_int32), C.c_int, _dp]
+        L.orc_hamiltonian.argtypes = [_c_int4, C.c_double, _dp, _dp, _dp, _dp]
+        L.orc_leapfrog.argtypes = [_c_int4, C.c_double, C.c_double, C.c_int, _dp, _dp]
+        L.orc_md_step.argtypes = [_c_int4, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_map.argtypes = [_c_int4, C.c_int, C.POINTER(C.c_int32)]
+        L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
+        L.orc_philox4x32_10.restype = None
+        for f in ("orc_herm_from_coeffs", "orc_expi"):
+            getattr(L, f).argtypes = [_dp, _dp]
+            getattr(L, f).restype = None
+        L.orc_reunit_mat.argtypes = [_dp]
+        L.orc_reunit_mat.restype = None
+
+    # ---- helpers
+    @staticmethod
+    def volume(dims):
+        return int(np.prod(dims))
+
+    def num_threads(self):
+        return int(self.lib.orc_num_threads())
+
+    @staticmethod
+    def _ok(rc, what):
+        if rc != 0:
+            raise ValueError(f"oracle {what} failed with code {rc}")
+
+    # ---- O1
+    def map(self, dims, which):
+        out = np.empty(self.volume(dims), dtype=np.int32)
+        self._ok(self.lib.orc_map(_c_int4(*dims), which, out.ctypes.data_as(C.POINTER(C.c_int32))), "map")
+        return out
+
+    # ---- O3
+    def philox(self, ctr, key):
+        c = (C.c_uint32 * 4)(*ctr)
+        k = (C.c_uint32 * 2)(*key)
+        o = (C.c_uint32 * 4)()
+        self.lib.orc_philox4x32_10(c, k, o)
+        return [int(x) for x in o]
+
+    def rng_block(self, seed, s, mu, j, stream_id, purpose):
+        w = (C.c_uint32 * 4)()
+        u = np.empty(2)
+        g = np.empty(2)
+        self.lib.orc_rng_block(seed, s, mu, j, stream_id, purpose, w, _ptr(u), _ptr(g))
+        return [int(x) for x in w], u, g
+
+    # ---- O2, O8, O9 single-matrix
+    def herm_from_coeffs(self, q):
+        q = np.ascontiguousarray(q, dtype=np.float64)
+        Q = np.empty((3, 3), dtype=np.complex128)
+        self.lib.orc_herm_from_coeffs(_ptr(q), _ptr(Q))
+        return Q
+
+    def expi(self, Q):
+        Q = np.ascontiguousarray(Q, dtype=np.complex128)
+        E = np.empty((3, 3), dtype=np.complex128)
+        self.lib.orc_expi(_ptr(Q), _ptr(E))
+        return E
+
+    def reunit_mat(self, M):
+        M = np.array(M, dtype=np.complex128, order="C")
+        self.lib.orc_reunit_mat(_ptr(M))
+        return M
+
+    # ---- O4, O5
+    def mom_refresh(self, dims, seed, stream_id=0, subset=ALL, out=None):
+        V = self.volume(dims)
+        P = np.zeros((V, 4, 3, 3), dtype=np.complex128) if out is None else out
+        self._ok(self.lib.orc_mom_refresh(_c_int4(*dims), subset, seed, stream_id, _mat(P, V)), "mom_refresh")
+        return P
+
+    def hot_start(self, dims, seed, sigma):
+        V = self.volume(dims)
+        U = np.empty((V, 4, 3, 3), dtype=np.complex128)
+        self._ok(self.lib.orc_hot_start(_c_int4(*dims), seed, sigma, _mat(U, V)), "hot_start")
+        return U
+
+    def perturb(self, dims, seed, sigma, U):
+        V = self.volume(dims)
+        U = U.copy()
+        self._ok(self.lib.orc_perturb(_c_int4(*dims), seed, sigma, _mat(U, V)), "perturb")
+        return U
+
+    def gauge_transform(self, dims, seed, sigma, U):
+        V = self.volume(dims)
+        G = np.empty((V, 3, 3), dtype=np.complex128)
+        Uo = np.empty_like(U)
+        self._ok(self.lib.orc_gauge_transform(_c_int4(*dims), seed, sigma, _mat(U, V), _ptr(G), _mat(Uo, V)),
+                 "gauge_transform")
+        return G, Uo
+
+    # ---- O6
+    def plaquette(self, dims, U):
+        V = self.volume(dims)
+        avg = np.empty(1)
+        per_t = np.empty(dims[3])
+        self._ok(self.lib.orc_plaquette(_c_int4(*dims), _mat(U, V), _ptr(avg), _ptr(per_t)), "plaquette")
+        return float(avg[0]), per_t
+
+    def action(self, dims, beta, U):
+        S = np.empty(1)
+        self._ok(self.lib.orc_action(_c_int4(*dims), beta, _mat(U, self.volume(dims)), _ptr(S)), "action")
+        return float(S[0])
+
+    def hamiltonian(self, dims, beta, U, P):
+        V = self.volume(dims)
+        K, S = np.empty(1), np.empty(1)
+        self._ok(self.lib.orc_hamiltonian(_c_int4(*dims), beta, _mat(U, V), _mat(P, V), _ptr(K), _ptr(S)), "H")
+        return float(K[0]), float(S[0])
+
+    # ---- O7
+    def gauge_force(self, dims, beta, U, subset=ALL, out=None):
+        V = self.volume(dims)
+        F = np.zeros_like(U) if out is None else out
+        self._ok(self.lib.orc_gauge_force(_c_int4(*dims), subset, beta, _mat(U, V), _mat(F, V)), "gauge_force")
+        return F
+
+    def sum_retr_w(self, dims, U):
+        out = np.empty(1)
+        self._ok(self.lib.orc_sum_retr_w(_c_int4(*dims), _mat(U, self.volume(dims)), _ptr(out)), "sum_retr_w")
+        return float(out[0])
+
+    # ---- O10 (in place on copies: inputs are never modified)
+    def mom_update(self, dims, eps, F, P, subset=ALL):
+        V = self.volume(dims)
+        P = P.copy()
+        self._ok(self.lib.orc_mom_update(_c_int4(*dims), subset, eps, _mat(F, V), _mat(P, V)), "mom_update")
+        return P
+
+    def link_update(self, dims, eps, P, U, reunit=False, subset=ALL):
+        V = self.volume(dims)
+        U = U.copy()
+        self._ok(self.lib.orc_link_update(_c_int4(*dims), subset, eps, _mat(P, V), _mat(U, V), int(reunit)),
+                 "link_update")
+        return U
+
+    def reunit(self, dims, U, subset=ALL):
+        V = self.volume(dims)
+        U = U.copy()
+        self._ok(self.lib.orc_reunit(_c_int4(*dims), subset, _mat(U, V)), "reunit")
+        return U
+
+    # ---- O12
+    def sum(self, dims, kind, field, subset=ALL):
+        V = self.volume(dims)
+        f = np.ascontiguousarray(field)
+        if f.dtype == np.complex128:
+            f = f.view(np.float64)
+        assert f.dtype == np.float64
+        f = f.reshape(V, -1)
+        ncomp = f.shape[1]
+        out = np.empty(ncomp if kind == SUM_SCALAR else 1)
+        self._ok(self.lib.orc_sum(_c_int4(*dims), subset, kind, ncomp, _ptr(f), _ptr(out)), "sum")
+        return out
+
+    def sum_multi(self, dims, kind, field, subset_id=None, nsub=None):
+        V = self.volume(dims)
+        f = np.ascontiguousarray(field)
+        if f.dtype == np.complex128:
+            f = f.view(np.float64)
+        f = f.reshape(V, -1)
+        ncomp = f.shape[1]
+        if subset_id is None:
+            nsub = dims[3]
+            idp = None
+        else:
+            subset_id = np.ascontiguousarray(subset_id, dtype=np.int32)
+            idp = subset_id.ctypes.data_as(C.POINTER(C.c_int32))
+        out = np.empty((nsub, ncomp) if kind == SUM_SCALAR else (nsub,))
+        self._ok(self.lib.orc_sum_multi(_c_int4(*dims), kind, ncomp, _ptr(f), idp, nsub, _ptr(out)), "sum_multi")
+        return out
+
+    # ---- O11
+    def leapfrog(self, dims, beta, eps, nsteps, U, P):
+        V = self.volume(dims)
+        U, P = U.copy(), P.copy()
+        self._ok(self.lib.orc_leapfrog(_c_int4(*dims), beta, eps, nsteps, _mat(U, V), _mat(P, V)), "leapfrog")
+        return U, P
+
+    def md_step(self, dims, beta, eps_p, eps_u, U, P, inplace=False):
+        V = self.volume(dims)
+        if not inplace:
+            U, P = U.copy(), P.copy()
+        self._ok(self.lib.orc_md_step(_c_int4(*dims), beta, eps_p, eps_u, _mat(U, V), _mat(P, V)), "md_step")
+        return U, P
