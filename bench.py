@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py — MD-step site-updates/s of the fused hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A "step" is one fused molecular-dynamics step on the whole lattice: qcd_force_mom_update
+(P += eps F(U)) then qcd_link_update with reunit (U <- reunit(exp(i eps P) U)) — both kernels of
+SURVEY.md section 8(a)'s "MD step (fused)" row.  Default workload: BASELINE config 4, 32^3x64 fp64,
+sigma=0.2, beta=6.0, eps=0.02, seeded synthetic hot start generated on the device.
+
+N > 1 (torchrun): the path is run as N independent replicas (one lattice per GPU, different seeds,
+no data-path collective); value = total site-updates/s, scaling "weak".
+
+--impl reference times the CPU oracle (oracle/, as it stands, serial) on a bounded sample of the
+same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+SEED_BASE = 0x1212078500000000
+CONFIGS = {  # BASELINE.json configs: dims, hot-start sigma, beta, eps
+    3: dict(dims=(16, 16, 16, 32), sigma=0.5, beta=5.8, eps=0.05, name="16^3x32"),
+    4: dict(dims=(32, 32, 32, 64), sigma=0.2, beta=6.0, eps=0.02, name="32^3x64"),
+    5: dict(dims=(48, 48, 48, 96), sigma=0.3, beta=6.2, eps=0.01, name="48^3x96"),
+}
+BYTES_PER_SITE = {"force_mom_update": 216, "link_update_reunit": 216}  # reals/site R+W
+METRIC = "md_step_site_updates_per_s"
+UNIT = "site-updates/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons through NVML (what nvidia-smi reads) while `active`"""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.mask, self.active, self.stop_flag = index, [], 0, False, False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # noqa: BLE001
+            self.nv, self.err = None, repr(e)
+
+    def run(self):
+        while not self.stop_flag and self.nv is not None:
+            if self.active:
+                try:
+                    self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                    self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:  # noqa: BLE001
+                    pass
+            time.sleep(0.005)
+
+    def summary(self):
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"], "samples": 0}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz,
+                "reasons": [n for b, n in self.REASONS.items() if self.mask & b], "samples": len(s)}
+
+
+def oracle_step_rate(orc, cfg, dims, steps, warmup):
+    """time `steps` fused MD steps of the oracle on lattice `dims` (same sigma, beta, eps as cfg)"""
+    seed = SEED_BASE + 4
+    U = orc.hot_start(dims, seed, cfg["sigma"])
+    P = orc.mom_refresh(dims, seed)
+    for _ in range(warmup):
+        orc.md_step(dims, cfg["beta"], cfg["eps"], cfg["eps"], U, P, inplace=True)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.md_step(dims, cfg["beta"], cfg["eps"], cfg["eps"], U, P, inplace=True)
+    dt = time.perf_counter() - t0
+    V = 1
+    for d in dims:
+        V *= d
+    return V * steps / dt, dt
+
+
+SAMPLE_LATTICES = [(4, 4, 4, 4), (8, 4, 4, 4), (8, 8, 4, 4), (8, 8, 8, 4), (8, 8, 8, 8), (16, 8, 8, 8), (16, 16, 8, 8),
+                   (16, 16, 16, 8), (16, 16, 16, 16), (32, 16, 16, 16), (32, 32, 16, 16), (32, 32, 32, 16)]
+
+
+def pick_sample(orc, cfg, steps_total, budget_s):
+    """largest sample lattice whose `steps_total` oracle steps fit the time budget"""
+    rate, _ = oracle_step_rate(orc, cfg, (8, 8, 8, 4), 1, 0)  # calibration, ~20 ms
+    best = SAMPLE_LATTICES[0]
+    for d in SAMPLE_LATTICES:
+        V = d[0] * d[1] * d[2] * d[3]
+        if V * steps_total / rate <= budget_s:
+            best = d
+    return best
+
+
+def run_reference(args, cfg):
+    """the oracle, as it stands (serial build), on the host cores; rank 0 only"""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle.oracle import Oracle
+    orc = Oracle(omp=False)
+    dims = pick_sample(orc, cfg, args.steps + args.warmup, 150.0)
+    rate, dt = oracle_step_rate(orc, cfg, dims, args.steps, args.warmup)
+    sample = (f"{'x'.join(map(str, dims))} lattice with the {cfg['name']} parameters (sigma={cfg['sigma']}, "
+              f"beta={cfg['beta']}, eps={cfg['eps']}), {args.steps} fused MD steps, serial C oracle")
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg['name']} fp64 fused MD step (bounded sample: {'x'.join(map(str, dims))})"},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1212_0785_b200 import binding as qcd
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dtype = torch.float64 if args.dtype == "f64" else torch.float32
+    rbytes = 8 if args.dtype == "f64" else 4
+    dims, beta, eps = cfg["dims"], cfg["beta"], cfg["eps"]
+    lat = qcd.Lattice(dims)
+    V = lat.V
+    U, P = lat.new_matrix_field(dtype), lat.new_matrix_field(dtype)
+    qcd.qcd_hot_start(lat, U, SEED_BASE + 4 + 1000 * rank, cfg["sigma"])
+    qcd.qcd_mom_refresh(lat, P, SEED_BASE + 4 + 1000 * rank)
+    stream = torch.cuda.current_stream()
+
+    for _ in range(args.warmup):
+        qcd.qcd_md_step(lat, U, P, beta, eps, eps)
+    try:  # NVML index of this CUDA device (differs from `local` under CUDA_VISIBLE_DEVICES)
+        nvml_index = torch.cuda._get_nvml_device_index(local)
+    except Exception:  # noqa: BLE001
+        nvml_index = local
+    sampler = ClockSampler(nvml_index)
+    sampler.start()
+
+    # ---- timed region: K fused MD steps, inputs resident in HBM (2 x field >> L2, see config.l2)
+    K = args.steps
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    barrier()
+    sampler.active = True
+    for k in range(K):
+        ev[k][0].record(stream)
+        qcd.qcd_force_mom_update(lat, U, P, beta, eps)
+        ev[k][1].record(stream)
+        qcd.qcd_link_update(lat, P, U, eps, reunit=True)
+        ev[k][2].record(stream)
+    barrier()
+    sampler.active = False
+    elapsed_ms = ev[0][0].elapsed_time(ev[K - 1][2])
+    force_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / K
+    link_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / K
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms = t.item()
+    value = world * V * K / (elapsed_ms * 1e-3)
+
+    # ---- e2e: the C-ABI call on HOST buffers (pinned), H2D + pack + step + unpack + D2H every step
+    Ke = max(1, min(K, args.e2e_steps))
+    fb = lat.field_bytes(qcd.F64 if args.dtype == "f64" else qcd.F32)
+    hU = torch.empty(V * 72, dtype=dtype).pin_memory()
+    hP = torch.empty(V * 72, dtype=dtype).pin_memory()
+    work = torch.empty(lat.md_host_work_bytes(qcd.F64 if args.dtype == "f64" else qcd.F32) // rbytes, dtype=dtype,
+                       device="cuda")
+    tmp = work[: V * 72]
+    qcd.qcd_unpack(lat, 72, U, tmp)
+    hU.copy_(tmp)
+    qcd.qcd_unpack(lat, 72, P, tmp)
+    hP.copy_(tmp)
+    qcd.qcd_md_host(lat, hU, hP, beta, eps, 1, work)  # warm-up
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(Ke):
+        qcd.qcd_md_host(lat, hU, hP, beta, eps, 1, work)
+        stream.synchronize()  # the caller reads the step's result on the host
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * V * Ke / (t.item() * 1e-3)
+    sampler.stop_flag = True
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = peaks()
+    force_bytes = BYTES_PER_SITE["force_mom_update"] * rbytes * V
+    achieved = force_bytes / (force_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(f"force_mom_update_{args.dtype}_{cfg['name']}")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": elapsed_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"{cfg['name']} {'fp64' if args.dtype == 'f64' else 'fp32'} fused MD step "
+                               f"(force+momentum, exp+reunit), sigma={cfg['sigma']} beta={beta} eps={eps}",
+                   "sites_per_gpu": V, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "l2": f"inputs U+P = {2 * fb / 1e6:.0f} MB per GPU, larger than the 126 MB L2: no flush needed"
+                         if 2 * fb > 2 * 126e6 else "inputs fit L2: numbers are L2-resident, not HBM",
+                   "step_hbm_gbs": 2 * force_bytes / (elapsed_ms / K * 1e-3) / 1e9,
+                   "step_frac_of_hbm_peak": 2 * force_bytes / (elapsed_ms / K * 1e-3) / 1e9 / peak,
+                   "kernel_ms": {"force_mom_update": force_ms, "link_update_reunit": link_ms}},
+        "roofline": {"bound": "hbm", "kernel": "force_mom_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": force_bytes},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * fb, "d2h_bytes_per_step": 2 * fb,
+                "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout)"},
+        "gpu_launches": 2 * K,
+        "clocks": sampler.summary(),
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle.oracle import Oracle
+        orc = Oracle(omp=False)
+        sd = pick_sample(orc, cfg, 6, 20.0)
+        rate, dt = oracle_step_rate(orc, cfg, sd, 5, 1)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                                "sample": f"{'x'.join(map(str, sd))} lattice with the {cfg['name']} parameters, "
+                                          f"5 fused MD steps of the serial C oracle ({dt:.1f} s)"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

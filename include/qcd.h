@@ -1,0 +1,193 @@
+/* qcd.h — C ABI of libqcdmd: B200 (sm_100a) kernels for the site-parallel SU(3) field operations of
+ * the Hybrid Monte-Carlo molecular-dynamics step outside the fermion inverter.
+ *
+ * The operations are the ones the paper lists as having to leave the CPU (section 1:
+ * "momentum updates, force term calculation, projection of fields, reunitarization of SU(3)
+ * matrices, a random number generator, exponentiating of SU(3) matrices") and its "non-linear
+ * algebra" reductions (section 1: "sum, sumMulti").  Every operation is site-parallel
+ * (Table 1 caption and section 3).  The paper defines none of them; the definitions
+ * are the textbook ones fixed in SURVEY.md section 8(c) and DESIGN.md ("Readings"), cited per call
+ * below as O1..O12.
+ *
+ * CONVENTIONS
+ *   Lattice: extents L = (Lx,Ly,Lz,Lt), all even and >= 2, V = Lx*Ly*Lz*Lt < 2^31, periodic.
+ *   Directions mu = 0..3 <-> x,y,z,t.  Lexicographic site index s = x + Lx*(y + Ly*(z + Lz*t)).
+ *   parity(s) = (x+y+z+t) & 1;  checkerboard index cb(s) = parity*V/2 + (s>>1).       [O1]
+ *
+ *   Precision `prec`: QCD_F64 fields are double, QCD_F32 fields are float.  All field arithmetic is
+ *   done in the field's precision; every reduction accumulates and returns double.
+ *
+ *   DEVICE layout of a matrix field (U, P, F; 4 links per site, 3x3 complex each = 72 reals/site):
+ *   checkerboarded, site-fastest structure of arrays of complex pairs.  Entry (mu, e = 3*row+col)
+ *   of site cb is the (re,im) pair at pair-index (mu*9 + e)*V + cb, i.e. a `double2`/`float2`
+ *   array of 36*V pairs.  Even sites are cb in [0,V/2), odd sites [V/2,V).
+ *   DEVICE layout of a real site field with ncomp components: real index comp*V + cb.
+ *   CANONICAL (exchange) layout, used by qcd_pack/qcd_unpack and the *_host call: lexicographic
+ *   array of structures [s][mu][row][col][re,im] (matrix) or [s][comp] (real).
+ *
+ *   Subsets: QCD_ALL, QCD_EVEN (parity 0), QCD_ODD.  A subset call writes only sites of the subset
+ *   and leaves every other site bit-identical; it may read any site.
+ *
+ * OWNERSHIP AND ASYNCHRONY
+ *   Unless a parameter says "host", every pointer is a DEVICE pointer owned by the caller (e.g. a
+ *   PyTorch tensor's data_ptr()).  The library allocates no device memory: fields, outputs and
+ *   workspace are the caller's and must stay alive until the stream work has completed.  `stream`
+ *   is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call only enqueues
+ *   work on `stream` and returns without synchronising; reduction results are written to device
+ *   doubles.  qcd_lattice is host-only, immutable after creation and may be shared across threads.
+ *
+ * ERRORS
+ *   Return code only: no exceptions, no abort, no printing.  On a nonzero return nothing was
+ *   enqueued.  qcd_last_error() returns a thread-local text for the last nonzero return.
+ *     QCD_EINVAL      NULL pointer, unknown enum value, nsub < 1, ncomp < 1 ...
+ *     QCD_EDIMS       an extent is odd or < 2, or V >= 2^31
+ *     QCD_EALIGN      a field pointer is not 16-byte aligned
+ *     QCD_EALIAS      input and output overlap where the operation forbids it
+ *     QCD_EWORKSPACE  reserved (workspace too small cannot be detected from a raw pointer)
+ *     QCD_ECUDA       the CUDA runtime reported a launch error (text in qcd_last_error)
+ *   Scalars beta, eps, sigma are double and rounded to float once for QCD_F32.
+ */
+#ifndef QCD_H
+#define QCD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qcd_lattice qcd_lattice; /* opaque, host side */
+
+enum { QCD_F32 = 0, QCD_F64 = 1 };
+enum { QCD_ALL = 0, QCD_EVEN = 1, QCD_ODD = 2 };
+enum { QCD_SUM_SCALAR = 0, QCD_SUM_NORM2 = 1, QCD_SUM_RETR = 2 };
+enum { QCD_OK = 0, QCD_EINVAL = 1, QCD_EDIMS = 2, QCD_EALIGN = 3, QCD_EALIAS = 4, QCD_EWORKSPACE = 5,
+       QCD_ECUDA = 6 };
+/* qcd_get_map `which`: maps are indexed by the lexicographic index and hold lexicographic indices,
+ * except CB_OF_LEX (value = checkerboard index) and LEX_OF_CB (indexed by checkerboard index). */
+enum { QCD_MAP_CB_OF_LEX = 0, QCD_MAP_LEX_OF_CB = 1, QCD_MAP_NBR_FWD0 = 2, QCD_MAP_NBR_FWD1 = 3,
+       QCD_MAP_NBR_FWD2 = 4, QCD_MAP_NBR_FWD3 = 5, QCD_MAP_NBR_BWD0 = 6, QCD_MAP_NBR_BWD1 = 7,
+       QCD_MAP_NBR_BWD2 = 8, QCD_MAP_NBR_BWD3 = 9, QCD_MAP_PARITY = 10, QCD_MAP_TSLICE = 11 };
+
+/* ---- lattice object, sizes, errors (host only; no CUDA call is made) ---------------------- */
+
+/* Create the host-side lattice descriptor for extents dims = (Lx,Ly,Lz,Lt).  [O1] */
+int qcd_lattice_create(const int dims[4], qcd_lattice **out);
+int qcd_lattice_destroy(qcd_lattice *lat);
+/* Number of sites V (0 if lat is NULL). */
+int64_t qcd_lattice_volume(const qcd_lattice *lat);
+/* Bytes of a device field with `ncomp_reals_per_site` reals per site (72 for U, P, F). */
+size_t qcd_field_bytes(const qcd_lattice *lat, int prec, int ncomp_reals_per_site);
+/* Bytes of the reduction workspace required by qcd_plaquette / qcd_sum / qcd_sum_multi /
+ * qcd_force_mom_update (when sums are requested). Depends only on the lattice. */
+size_t qcd_workspace_bytes(const qcd_lattice *lat);
+/* Device bytes needed by qcd_md_host (staging + fields). */
+size_t qcd_md_host_work_bytes(const qcd_lattice *lat, int prec);
+const char *qcd_last_error(void);
+/* Library version string, e.g. "qcdmd 0.1 sm_100a". */
+const char *qcd_version(void);
+
+/* ---- the hot path ----------------------------------------------------------- */
+
+/* Wilson gauge force [O7]: for every site of `subset` and every mu
+ *   A = sum_{nu!=mu} [ U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag + U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu) ]
+ *   W = U_mu(x) A ;  F_mu(x) = (i beta/12) [ (W - W^dag) - (1/3) tr(W - W^dag) ]      ("force term
+ *   calculation", "projection of fields").  F Hermitian traceless; with dU/dt = iPU, dP/dt = F
+ *   conserves H = sum tr P^2 + beta sum_{x,mu<nu} (1 - (1/3) Re tr P_mu_nu(x)).
+ * U: matrix field, read at all sites.  F: matrix field, written on the subset.  U and F must not
+ * overlap (QCD_EALIAS). */
+int qcd_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, const void *U, void *F,
+                    void *stream);
+
+/* Momentum update [O10]: P <- P + eps*F on the subset ("momentum updates"). F and P must not overlap. */
+int qcd_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P,
+                   void *stream);
+
+/* Fused force + momentum update (the loop fusion of PAPER.md:32): P <- P + eps*F(U) on the subset,
+ * F never stored.  U and P must not overlap. */
+int qcd_force_mom_update(const qcd_lattice *lat, int prec, int subset, double beta, double eps,
+                         const void *U, void *P, void *stream);
+
+/* Link update [O8,O10]: U_mu(x) <- exp(i eps P_mu(x)) U_mu(x) on the subset ("exponentiating of
+ * SU(3) matrices"); exp is exact to rounding for Hermitian traceless P of any norm.  If reunit != 0
+ * the result is reunitarised in registers as by qcd_reunit before it is stored.  P and U must not
+ * overlap. */
+int qcd_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,
+                    int reunit, void *stream);
+
+/* Reunitarisation [O9] on the subset, in place ("reunitarization of SU(3) matrices"): rows r0,r1,r2:
+ * r0 <- r0/|r0| ; r1 <- r1 - (r0^dag.r1) r0, r1 <- r1/|r1| ; r2 <- conj(r0 x r1). */
+int qcd_reunit(const qcd_lattice *lat, int prec, int subset, void *U, void *stream);
+
+/* Gaussian momentum refresh [O3,O4] on the subset ("a random number generator"): for each link the
+ * eight coefficients p_a ~ N(0,1) of P = sum_a p_a T_a (T_a = Gell-Mann/2) come from the counter-based
+ * generator Philox4x32-10 with key = seed and counter (lexicographic site, mu*16+j, stream_id,
+ * purpose=1), j = 0..3, two Box-Muller outputs per block.  The result does not depend on the subset,
+ * the layout or the launch shape. */
+int qcd_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id,
+                    void *P, void *stream);
+
+/* Plaquette [O6] ("sum", "sumMulti"): out_avg[0] = (1/6V) sum_x sum_{mu<nu} (1/3) Re tr P_mu_nu(x),
+ * P_mu_nu(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag, and, if out_per_t != NULL, the same
+ * average over each timeslice (a plaquette belongs to the timeslice of its base site x), Lt doubles.
+ * Deterministic: fixed two-pass reduction order, bit-identical from run to run.
+ * out_avg, out_per_t: device doubles.  workspace: qcd_workspace_bytes(lat) device bytes. */
+int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                  void *workspace, void *stream);
+
+/* Global / subset sum [O12] ("sum") of a per-site quantity of `field`:
+ *   QCD_SUM_SCALAR  real field with ncomp components: out[c] = sum_x field_c(x), c < ncomp <= 64
+ *   QCD_SUM_NORM2   field with ncomp reals per site (ncomp even): out[0] = sum_x sum_i field_i(x)^2
+ *                   (ncomp = 72 on P gives the kinetic energy sum tr P^2)
+ *   QCD_SUM_RETR    matrix field of ncomp/18 matrices per site: out[0] = sum_x sum_m Re tr M_m(x)
+ * Deterministic two-pass reduction in double.  out: device doubles. */
+int qcd_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, const void *field,
+            double *out, void *workspace, void *stream);
+
+/* Per-subset sums [O12] ("sumMulti"): out[k] (SCALAR: out[k*ncomp + c]) = sum over the sites with
+ * subset_id == k.  subset_id: device int32[V] indexed by CHECKERBOARD index with values in [0,nsub)
+ * (other values: site belongs to no subset), or NULL for the timeslice set (nsub must equal Lt).
+ * nsub <= 4096.  Deterministic. */
+int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
+                  const int32_t *subset_id, int nsub, double *out, void *workspace, void *stream);
+
+/* One fused MD step, the unit the headline metric counts: P <- P + eps_p*F(U), then
+ * U <- reunit(exp(i eps_u P) U), two kernels on `stream`. [O11 building block] */
+int qcd_md_step(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, void *U,
+                void *P, void *stream);
+
+/* Leapfrog trajectory [O11]: P += (eps/2) F; n times { U <- reunit(exp(i eps P) U); P += eps F }
+ * with eps/2 on the last. */
+int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,
+                 void *P, void *stream);
+
+/* ---- helpers (not on the hot path) -------------------------------------------------------- */
+
+/* canonical lexicographic AoS (device) -> device layout, and back. ncomp reals per site, even. For
+ * matrix fields ncomp = 72.  Input and output must not overlap. */
+int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream);
+int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa, void *lex_aos, void *stream);
+/* index / subset maps [O1] into dev_out (int32[V]) */
+int qcd_get_map(const qcd_lattice *lat, int which, int32_t *dev_out, void *stream);
+/* hot start [O5]: U_mu(x) = exp(i sigma Q), Q = sum q_a T_a, q_a ~ N(0,1) from purpose 0 */
+int qcd_hot_start(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, void *stream);
+/* U += sigma*N, 18 iid N(0,1) reals per link from purpose 2, blocks 0..8 (config 3 reunit input) */
+int qcd_perturb(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, void *stream);
+/* raw generator output for bit-exact tests: for i < n, block counter (site[i], mu_j[i], stream_id,
+ * purpose) -> words[4*i..4*i+3] (uint32), uniforms[2*i..] (double), gauss[2*i..] (double).
+ * site, mu_j: device uint32[n]; any output pointer may be NULL. */
+int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, const uint32_t *site,
+                   const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, void *stream);
+
+/* End-to-end call on HOST buffers (used for the e2e measurement): U_host and P_host are host arrays
+ * in the canonical layout (pinned memory makes the copies asynchronous).  Enqueues on `stream`:
+ * host->device copies, pack, `nsteps` fused MD steps (eps_p = eps_u = eps), unpack, device->host
+ * copies back into U_host and P_host.  device_work: qcd_md_host_work_bytes(lat, prec) device bytes. */
+int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host,
+                void *P_host, void *device_work, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCD_H */

@@ -48,6 +48,7 @@ class Oracle:
         L.orc_plaquette.argtypes = [_c_int4, _dp, _dp, _dp]
         L.orc_action.argtypes = [_c_int4, C.c_double, _dp, _dp]
         L.orc_gauge_force.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp]
+        L.orc_gauge_force_sites.argtypes = [_c_int4, C.c_double, _dp, C.c_int, C.POINTER(C.c_int32), _dp]
         L.orc_sum_retr_w.argtypes = [_c_int4, _dp, _dp]
         L.orc_mom_update.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp]
         L.orc_link_update.argtypes = [_c_int4, C.c_int, C.c_double, _dp, _dp, C.c_int]
@@ -169,6 +170,14 @@ class Oracle:
         V = self.volume(dims)
         F = np.zeros_like(U) if out is None else out
         self._ok(self.lib.orc_gauge_force(_c_int4(*dims), subset, beta, _mat(U, V), _mat(F, V)), "gauge_force")
+        return F
+
+    def gauge_force_sites(self, dims, beta, U, sites):
+        sites = np.ascontiguousarray(sites, dtype=np.int32)
+        F = np.empty((len(sites), 4, 3, 3), dtype=np.complex128)
+        self._ok(self.lib.orc_gauge_force_sites(_c_int4(*dims), beta, _mat(U, self.volume(dims)), len(sites),
+                                                sites.ctypes.data_as(C.POINTER(C.c_int32)), _ptr(F)),
+                 "gauge_force_sites")
         return F
 
     def sum_retr_w(self, dims, U):

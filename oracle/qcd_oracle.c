@@ -447,6 +447,20 @@ int orc_gauge_force(const int L[4], int subset, double beta, const double *U, do
     return 0;
 }
 
+/* the same force_link at a list of sites only (sampled parity on the large lattices);
+ * F is double[nsites][4][3][3][2] */
+int orc_gauge_force_sites(const int L[4], double beta, const double *U, int nsites, const int32_t *sites,
+                          double *F) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !U || !F || nsites < 0 || (nsites && !sites)) return 1;
+    for (int i = 0; i < nsites; i++)
+        if (sites[i] < 0 || sites[i] >= lat.V) return 1;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < nsites; i++)
+        for (int mu = 0; mu < 4; mu++) force_link(&lat, beta, U, sites[i], mu, LINK(F, i, mu));
+    return 0;
+}
+
 int orc_sum_retr_w(const int L[4], const double *U, double *out) {
     lat_t lat;
     if (lat_init(&lat, L) || !U || !out) return 1;

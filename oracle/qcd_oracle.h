@@ -62,6 +62,9 @@ int orc_plaquette(const int L[4], const double *U, double *avg, double *per_t /*
 int orc_action(const int L[4], double beta, const double *U, double *S);
 /* O7 */
 int orc_gauge_force(const int L[4], int subset, double beta, const double *U, double *F);
+/* O7 at the listed lexicographic sites only; F is double[nsites][4][3][3][2] */
+int orc_gauge_force_sites(const int L[4], double beta, const double *U, int nsites, const int32_t *sites,
+                          double *F);
 /* pin helper: sum over x,mu of Re tr W_mu(x), W = U_mu(x) A_mu(x) (staple sum rule) */
 int orc_sum_retr_w(const int L[4], const double *U, double *out);
 /* O10 */

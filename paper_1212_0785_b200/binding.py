@@ -1,0 +1,233 @@
+"""Thin Python binding of the C ABI in include/qcd.h (same names, argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libqcdmd.so; PyTorch is used for device memory
+(tensors), streams and nothing else.  There is no CPU fallback: if the library is missing the import
+fails loudly.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqcdmd.so")
+
+F32, F64 = 0, 1
+ALL, EVEN, ODD = 0, 1, 2
+SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
+OK, EINVAL, EDIMS, EALIGN, EALIAS, EWORKSPACE, ECUDA = range(7)
+MAP_CB_OF_LEX, MAP_LEX_OF_CB, MAP_NBR_FWD0, MAP_NBR_BWD0, MAP_PARITY, MAP_TSLICE = 0, 1, 2, 6, 10, 11
+
+# every symbol include/qcd.h declares, with its ctypes signature (restype, argtypes)
+_vp, _i, _d, _u64, _u32, _sz = C.c_void_p, C.c_int, C.c_double, C.c_uint64, C.c_uint32, C.c_size_t
+SIGNATURES = {
+    "qcd_lattice_create": (_i, [C.POINTER(C.c_int * 4), C.POINTER(_vp)]),
+    "qcd_lattice_destroy": (_i, [_vp]),
+    "qcd_lattice_volume": (C.c_int64, [_vp]),
+    "qcd_field_bytes": (_sz, [_vp, _i, _i]),
+    "qcd_workspace_bytes": (_sz, [_vp]),
+    "qcd_md_host_work_bytes": (_sz, [_vp, _i]),
+    "qcd_last_error": (C.c_char_p, []),
+    "qcd_version": (C.c_char_p, []),
+    "qcd_gauge_force": (_i, [_vp, _i, _i, _d, _vp, _vp, _vp]),
+    "qcd_mom_update": (_i, [_vp, _i, _i, _d, _vp, _vp, _vp]),
+    "qcd_force_mom_update": (_i, [_vp, _i, _i, _d, _d, _vp, _vp, _vp]),
+    "qcd_link_update": (_i, [_vp, _i, _i, _d, _vp, _vp, _i, _vp]),
+    "qcd_reunit": (_i, [_vp, _i, _i, _vp, _vp]),
+    "qcd_mom_refresh": (_i, [_vp, _i, _i, _u64, _u32, _vp, _vp]),
+    "qcd_plaquette": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_sum": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp]),
+    "qcd_sum_multi": (_i, [_vp, _i, _i, _i, _vp, _vp, _i, _vp, _vp, _vp]),
+    "qcd_md_step": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp]),
+    "qcd_leapfrog": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp]),
+    "qcd_pack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
+    "qcd_unpack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
+    "qcd_get_map": (_i, [_vp, _i, _vp, _vp]),
+    "qcd_hot_start": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
+    "qcd_perturb": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
+    "qcd_rng_blocks": (_i, [_u64, _u32, _u32, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_md_host": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
+}
+
+
+def load_library(path=LIB_PATH):
+    if not os.path.exists(path):
+        raise ImportError(
+            f"{path} is missing: build it with `python -m paper_1212_0785_b200.build` "
+            "(there is no CPU fallback for the CUDA path)")
+    lib = C.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)  # AttributeError if the library does not export a declared symbol
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+lib = load_library()
+
+
+class QcdError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"qcd error {code}: {text}")
+        self.code = code
+
+
+def _check(rc):
+    if rc != OK:
+        raise QcdError(rc, lib.qcd_last_error().decode())
+
+
+def _prec(t):
+    if t.dtype == torch.float64:
+        return F64
+    if t.dtype == torch.float32:
+        return F32
+    raise TypeError(f"field dtype must be float32 or float64, got {t.dtype}")
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+class Lattice:
+    """qcd_lattice handle (host side)."""
+
+    def __init__(self, dims):
+        self.dims = tuple(int(d) for d in dims)
+        h = _vp()
+        arr = (C.c_int * 4)(*self.dims) if len(self.dims) == 4 else None
+        if arr is None:
+            raise QcdError(EINVAL, "dims must have 4 entries")
+        _check(lib.qcd_lattice_create(C.byref(arr), C.byref(h)))
+        self.handle = h
+        self.V = int(lib.qcd_lattice_volume(h))
+
+    def __del__(self):
+        h = getattr(self, "handle", None)
+        if h:
+            lib.qcd_lattice_destroy(h)
+            self.handle = None
+
+    def field_bytes(self, prec, ncomp=72):
+        return int(lib.qcd_field_bytes(self.handle, prec, ncomp))
+
+    def workspace_bytes(self):
+        return int(lib.qcd_workspace_bytes(self.handle))
+
+    def md_host_work_bytes(self, prec):
+        return int(lib.qcd_md_host_work_bytes(self.handle, prec))
+
+    # ---- device memory (PyTorch owns it)
+    def new_matrix_field(self, dtype=torch.float64, device="cuda"):
+        """[36][V][2]: entry (mu*9+e, cb, re/im)"""
+        return torch.empty((36, self.V, 2), dtype=dtype, device=device)
+
+    def new_real_field(self, ncomp, dtype=torch.float64, device="cuda"):
+        return torch.empty((ncomp, self.V), dtype=dtype, device=device)
+
+    def new_workspace(self, device="cuda"):
+        return torch.empty(self.workspace_bytes() // 8, dtype=torch.float64, device=device)
+
+
+# ---- the calls, named as in include/qcd.h ---------------------------------------------------
+
+def qcd_gauge_force(lat, U, F, beta, subset=ALL, stream=None):
+    _check(lib.qcd_gauge_force(lat.handle, _prec(U), subset, beta, _ptr(U), _ptr(F), _stream(stream)))
+
+
+def qcd_mom_update(lat, F, P, eps, subset=ALL, stream=None):
+    _check(lib.qcd_mom_update(lat.handle, _prec(P), subset, eps, _ptr(F), _ptr(P), _stream(stream)))
+
+
+def qcd_force_mom_update(lat, U, P, beta, eps, subset=ALL, stream=None):
+    _check(lib.qcd_force_mom_update(lat.handle, _prec(U), subset, beta, eps, _ptr(U), _ptr(P), _stream(stream)))
+
+
+def qcd_link_update(lat, P, U, eps, reunit=False, subset=ALL, stream=None):
+    _check(lib.qcd_link_update(lat.handle, _prec(U), subset, eps, _ptr(P), _ptr(U), int(reunit), _stream(stream)))
+
+
+def qcd_reunit(lat, U, subset=ALL, stream=None):
+    _check(lib.qcd_reunit(lat.handle, _prec(U), subset, _ptr(U), _stream(stream)))
+
+
+def qcd_mom_refresh(lat, P, seed, stream_id=0, subset=ALL, stream=None):
+    _check(lib.qcd_mom_refresh(lat.handle, _prec(P), subset, seed, stream_id, _ptr(P), _stream(stream)))
+
+
+def qcd_plaquette(lat, U, out_avg, out_per_t, workspace, stream=None):
+    _check(lib.qcd_plaquette(lat.handle, _prec(U), _ptr(U), _ptr(out_avg), _ptr(out_per_t), _ptr(workspace),
+                             _stream(stream)))
+
+
+def qcd_sum(lat, kind, ncomp, field, out, workspace, subset=ALL, stream=None):
+    _check(lib.qcd_sum(lat.handle, _prec(field), subset, kind, ncomp, _ptr(field), _ptr(out), _ptr(workspace),
+                       _stream(stream)))
+
+
+def qcd_sum_multi(lat, kind, ncomp, field, subset_id, nsub, out, workspace, stream=None):
+    _check(lib.qcd_sum_multi(lat.handle, _prec(field), kind, ncomp, _ptr(field), _ptr(subset_id), nsub, _ptr(out),
+                             _ptr(workspace), _stream(stream)))
+
+
+def qcd_md_step(lat, U, P, beta, eps_p, eps_u, stream=None):
+    _check(lib.qcd_md_step(lat.handle, _prec(U), beta, eps_p, eps_u, _ptr(U), _ptr(P), _stream(stream)))
+
+
+def qcd_leapfrog(lat, U, P, beta, eps, nsteps, stream=None):
+    _check(lib.qcd_leapfrog(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _stream(stream)))
+
+
+def qcd_pack(lat, ncomp, lex_aos, dev_soa, stream=None):
+    _check(lib.qcd_pack(lat.handle, _prec(dev_soa), ncomp, _ptr(lex_aos), _ptr(dev_soa), _stream(stream)))
+
+
+def qcd_unpack(lat, ncomp, dev_soa, lex_aos, stream=None):
+    _check(lib.qcd_unpack(lat.handle, _prec(dev_soa), ncomp, _ptr(dev_soa), _ptr(lex_aos), _stream(stream)))
+
+
+def qcd_get_map(lat, which, out, stream=None):
+    _check(lib.qcd_get_map(lat.handle, which, _ptr(out), _stream(stream)))
+
+
+def qcd_hot_start(lat, U, seed, sigma, stream=None):
+    _check(lib.qcd_hot_start(lat.handle, _prec(U), seed, sigma, _ptr(U), _stream(stream)))
+
+
+def qcd_perturb(lat, U, seed, sigma, stream=None):
+    _check(lib.qcd_perturb(lat.handle, _prec(U), seed, sigma, _ptr(U), _stream(stream)))
+
+
+def qcd_rng_blocks(seed, stream_id, purpose, site, mu_j, words=None, uniforms=None, gauss=None, stream=None):
+    _check(lib.qcd_rng_blocks(seed, stream_id, purpose, site.numel(), _ptr(site), _ptr(mu_j), _ptr(words),
+                              _ptr(uniforms), _ptr(gauss), _stream(stream)))
+
+
+def qcd_md_host(lat, U_host, P_host, beta, eps, nsteps, device_work, stream=None):
+    """U_host, P_host: host tensors (pinned for asynchronous copies) in the canonical layout [V,4,3,3,2]."""
+    _check(lib.qcd_md_host(lat.handle, _prec(U_host), beta, eps, nsteps, _ptr(U_host), _ptr(P_host),
+                           _ptr(device_work), _stream(stream)))
+
+
+# ---- convenience used by tests and bench: canonical host arrays <-> device fields (via qcd_pack) ----
+
+def field_to_device(lat, host_array, dtype=torch.float64):
+    """numpy complex128 [V,4,3,3] (canonical layout) -> device matrix field of `dtype`"""
+    t = torch.view_as_real(torch.from_numpy(host_array)).reshape(-1).to(dtype).cuda()
+    out = lat.new_matrix_field(dtype)
+    qcd_pack(lat, 72, t, out)
+    torch.cuda.current_stream().synchronize()
+    return out
+
+
+def field_to_host(lat, dev_field):
+    """device matrix field -> numpy complex128 [V,4,3,3]"""
+    t = torch.empty(lat.V * 72, dtype=dev_field.dtype, device=dev_field.device)
+    qcd_unpack(lat, 72, dev_field, t)
+    return t.to(torch.float64).cpu().numpy().view("complex128").reshape(lat.V, 4, 3, 3)

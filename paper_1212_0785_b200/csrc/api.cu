@@ -1,0 +1,328 @@
+// api.cu — the C ABI of include/qcd.h: argument checks, error text, dispatch to the kernel launchers.
+#include <cstdarg>
+#include <cstdio>
+#include <new>
+
+#include "qcd_internal.h"
+#include "site.cuh"
+
+namespace qcd {
+
+static thread_local char g_err[256] = "";
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+int check_launch(const char *what) {
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_error("%s: %s", what, cudaGetErrorString(e));
+        return QCD_ECUDA;
+    }
+    return QCD_OK;
+}
+
+static size_t real_bytes(int prec) { return prec == QCD_F64 ? 8 : 4; }
+
+static int bad(int code, const char *fmt, const char *a = "") {
+    set_error(fmt, a);
+    return code;
+}
+
+static int check_common(const qcd_lattice *lat, int prec, const char *fn) {
+    if (!lat) return bad(QCD_EINVAL, "%s: lattice is NULL", fn);
+    if (prec != QCD_F32 && prec != QCD_F64) return bad(QCD_EINVAL, "%s: unknown prec", fn);
+    return QCD_OK;
+}
+static int check_subset(int subset, const char *fn) {
+    if (subset != QCD_ALL && subset != QCD_EVEN && subset != QCD_ODD) return bad(QCD_EINVAL, "%s: unknown subset", fn);
+    return QCD_OK;
+}
+static int check_ptr(const void *p, const char *fn) {
+    if (!p) return bad(QCD_EINVAL, "%s: NULL field pointer", fn);
+    if (((uintptr_t)p) & 15) return bad(QCD_EALIGN, "%s: field pointer not 16-byte aligned", fn);
+    return QCD_OK;
+}
+static int check_alias(const void *a, const void *b, size_t bytes, const char *fn) {
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    if (x < y + bytes && y < x + bytes) return bad(QCD_EALIAS, "%s: input and output fields overlap", fn);
+    return QCD_OK;
+}
+
+}  // namespace qcd
+
+using namespace qcd;
+
+#define QCD_TRY(expr)            \
+    do {                         \
+        const int rc_ = (expr);  \
+        if (rc_ != QCD_OK) return rc_; \
+    } while (0)
+
+extern "C" {
+
+int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
+    if (!dims || !out) return bad(QCD_EINVAL, "%s: NULL argument", "qcd_lattice_create");
+    long long V = 1;
+    for (int d = 0; d < 4; d++) {
+        if (dims[d] < 2 || (dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", "qcd_lattice_create");
+        V *= dims[d];
+        if (V >= (1ll << 31)) return bad(QCD_EDIMS, "%s: V must be < 2^31", "qcd_lattice_create");
+    }
+    qcd_lattice *lat = new (std::nothrow) qcd_lattice;
+    if (!lat) return bad(QCD_EINVAL, "%s: out of host memory", "qcd_lattice_create");
+    int stride = 1;
+    for (int d = 0; d < 4; d++) {
+        lat->p.L[d] = dims[d];
+        lat->p.stride[d] = stride;
+        stride *= dims[d];
+    }
+    lat->p.V = (int)V;
+    lat->p.Vh = (int)(V / 2);
+    const int Vsh = lat->p.Vh / dims[3];
+    lat->red_chunks_per_seg = (Vsh + RED_CHUNK - 1) / RED_CHUNK;
+    lat->red_nseg = 2 * dims[3];
+    const size_t a = (size_t)MAX_SUM_NCOMP * lat->red_nseg * lat->red_chunks_per_seg;
+    const size_t b = (size_t)MAX_NSUB * RED_GENERIC_CHUNKS;
+    lat->workspace_doubles = (a > b ? a : b) + 64;
+    *out = lat;
+    return QCD_OK;
+}
+
+int qcd_lattice_destroy(qcd_lattice *lat) {
+    delete lat;
+    return QCD_OK;
+}
+
+int64_t qcd_lattice_volume(const qcd_lattice *lat) { return lat ? lat->p.V : 0; }
+
+size_t qcd_field_bytes(const qcd_lattice *lat, int prec, int ncomp) {
+    if (!lat || ncomp < 1 || (prec != QCD_F32 && prec != QCD_F64)) return 0;
+    return (size_t)lat->p.V * ncomp * real_bytes(prec);
+}
+
+size_t qcd_workspace_bytes(const qcd_lattice *lat) { return lat ? lat->workspace_doubles * sizeof(double) : 0; }
+
+size_t qcd_md_host_work_bytes(const qcd_lattice *lat, int prec) { return 4 * qcd_field_bytes(lat, prec, 72); }
+
+const char *qcd_last_error(void) { return g_err; }
+
+const char *qcd_version(void) { return "qcdmd 0.1 sm_100a"; }
+
+int qcd_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, const void *U, void *F, void *stream) {
+    const char *fn = "qcd_gauge_force";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(F, fn));
+    QCD_TRY(check_alias(U, F, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_gauge_force(lat, prec, subset, beta, 0.0, U, F, false, (cudaStream_t)stream);
+}
+
+int qcd_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P, void *stream) {
+    const char *fn = "qcd_mom_update";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(F, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(F, P, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_mom_update(lat, prec, subset, eps, F, P, (cudaStream_t)stream);
+}
+
+int qcd_force_mom_update(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
+                         void *P, void *stream) {
+    const char *fn = "qcd_force_mom_update";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_gauge_force(lat, prec, subset, beta, eps, U, P, true, (cudaStream_t)stream);
+}
+
+int qcd_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U, int reunit,
+                    void *stream) {
+    const char *fn = "qcd_link_update";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_alias(P, U, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_link_update(lat, prec, subset, eps, P, U, reunit ? 1 : 0, (cudaStream_t)stream);
+}
+
+int qcd_reunit(const qcd_lattice *lat, int prec, int subset, void *U, void *stream) {
+    const char *fn = "qcd_reunit";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(U, fn));
+    return launch_link_update(lat, prec, subset, 0.0, U, U, 2, (cudaStream_t)stream);
+}
+
+int qcd_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *P,
+                    void *stream) {
+    const char *fn = "qcd_mom_refresh";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(P, fn));
+    return launch_mom_refresh(lat, prec, subset, seed, stream_id, P, (cudaStream_t)stream);
+}
+
+int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                  void *workspace, void *stream) {
+    const char *fn = "qcd_plaquette";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    if (!out_avg || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    return launch_plaquette(lat, prec, U, out_avg, out_per_t, (double *)workspace, (cudaStream_t)stream);
+}
+
+static int check_sum_args(int kind, int ncomp, const char *fn) {
+    if (kind != QCD_SUM_SCALAR && kind != QCD_SUM_NORM2 && kind != QCD_SUM_RETR) return bad(QCD_EINVAL, "%s: unknown kind", fn);
+    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    if (kind == QCD_SUM_SCALAR && ncomp > MAX_SUM_NCOMP) return bad(QCD_EINVAL, "%s: ncomp > 64 for SCALAR", fn);
+    if (kind != QCD_SUM_SCALAR && ncomp % 18) return bad(QCD_EINVAL, "%s: matrix kinds need ncomp %% 18 == 0", fn);
+    return QCD_OK;
+}
+
+int qcd_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, const void *field, double *out,
+            void *workspace, void *stream) {
+    const char *fn = "qcd_sum";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_sum_args(kind, ncomp, fn));
+    QCD_TRY(check_ptr(field, fn));
+    if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    return launch_sum(lat, prec, subset, kind, ncomp, field, out, (double *)workspace, (cudaStream_t)stream);
+}
+
+int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field, const int32_t *subset_id,
+                  int nsub, double *out, void *workspace, void *stream) {
+    const char *fn = "qcd_sum_multi";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_sum_args(kind, ncomp, fn));
+    QCD_TRY(check_ptr(field, fn));
+    if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    if (nsub < 1 || nsub > MAX_NSUB) return bad(QCD_EINVAL, "%s: nsub out of range [1,4096]", fn);
+    if (!subset_id && nsub != lat->p.L[3]) return bad(QCD_EINVAL, "%s: timeslice set needs nsub == Lt", fn);
+    if (subset_id && (size_t)nsub * (kind == QCD_SUM_SCALAR ? ncomp : 1) > (size_t)MAX_NSUB)
+        return bad(QCD_EINVAL, "%s: nsub*ncomp > 4096 on the subset_id path", fn);
+    return launch_sum_multi(lat, prec, kind, ncomp, field, subset_id, nsub, out, (double *)workspace,
+                            (cudaStream_t)stream);
+}
+
+int qcd_md_step(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, void *U, void *P,
+                void *stream) {
+    const char *fn = "qcd_md_step";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps_p, U, P, true, (cudaStream_t)stream));
+    return launch_link_update(lat, prec, QCD_ALL, eps_u, P, U, 1, (cudaStream_t)stream);
+}
+
+int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
+                 void *stream) {
+    const char *fn = "qcd_leapfrog";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    if (nsteps < 1) return bad(QCD_EINVAL, "%s: nsteps < 1", fn);
+    cudaStream_t st = (cudaStream_t)stream;
+    QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, U, P, true, st));
+    for (int k = 0; k < nsteps; k++) {
+        QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
+        QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, k == nsteps - 1 ? 0.5 * eps : eps, U, P, true, st));
+    }
+    return QCD_OK;
+}
+
+int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream) {
+    const char *fn = "qcd_pack";
+    QCD_TRY(check_common(lat, prec, fn));
+    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    QCD_TRY(check_ptr(lex_aos, fn));
+    QCD_TRY(check_ptr(dev_soa, fn));
+    QCD_TRY(check_alias(lex_aos, dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
+    return launch_pack(lat, prec, ncomp, lex_aos, dev_soa, false, (cudaStream_t)stream);
+}
+
+int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa, void *lex_aos, void *stream) {
+    const char *fn = "qcd_unpack";
+    QCD_TRY(check_common(lat, prec, fn));
+    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    QCD_TRY(check_ptr(lex_aos, fn));
+    QCD_TRY(check_ptr(dev_soa, fn));
+    QCD_TRY(check_alias(lex_aos, dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
+    return launch_pack(lat, prec, ncomp, dev_soa, lex_aos, true, (cudaStream_t)stream);
+}
+
+int qcd_get_map(const qcd_lattice *lat, int which, int32_t *dev_out, void *stream) {
+    const char *fn = "qcd_get_map";
+    if (!lat || !dev_out) return bad(QCD_EINVAL, "%s: NULL argument", fn);
+    if (which < QCD_MAP_CB_OF_LEX || which > QCD_MAP_TSLICE) return bad(QCD_EINVAL, "%s: unknown map", fn);
+    return launch_get_map(lat, which, dev_out, (cudaStream_t)stream);
+}
+
+int qcd_hot_start(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, void *stream) {
+    const char *fn = "qcd_hot_start";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    return launch_hot_start(lat, prec, seed, sigma, U, (cudaStream_t)stream);
+}
+
+int qcd_perturb(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, void *stream) {
+    const char *fn = "qcd_perturb";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    return launch_perturb(lat, prec, seed, sigma, U, (cudaStream_t)stream);
+}
+
+int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, const uint32_t *site,
+                   const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, void *stream) {
+    const char *fn = "qcd_rng_blocks";
+    if (n < 0 || (n > 0 && (!site || !mu_j))) return bad(QCD_EINVAL, "%s: bad arguments", fn);
+    return launch_rng_blocks(seed, stream_id, purpose, n, site, mu_j, words, uniforms, gauss, (cudaStream_t)stream);
+}
+
+int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host, void *P_host,
+                void *device_work, void *stream) {
+    const char *fn = "qcd_md_host";
+    QCD_TRY(check_common(lat, prec, fn));
+    if (!U_host || !P_host) return bad(QCD_EINVAL, "%s: NULL host buffer", fn);
+    QCD_TRY(check_ptr(device_work, fn));
+    if (nsteps < 0) return bad(QCD_EINVAL, "%s: nsteps < 0", fn);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    char *w = (char *)device_work;
+    void *stageU = w, *stageP = w + fb, *U = w + 2 * fb, *P = w + 3 * fb;
+    cudaError_t e = cudaMemcpyAsync(stageU, U_host, fb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(stageP, P_host, fb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) {
+        set_error("%s: H2D copy: %s", fn, cudaGetErrorString(e));
+        return QCD_ECUDA;
+    }
+    QCD_TRY(launch_pack(lat, prec, 72, stageU, U, false, st));
+    QCD_TRY(launch_pack(lat, prec, 72, stageP, P, false, st));
+    for (int k = 0; k < nsteps; k++) {
+        QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps, U, P, true, st));
+        QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
+    }
+    QCD_TRY(launch_pack(lat, prec, 72, U, stageU, true, st));
+    QCD_TRY(launch_pack(lat, prec, 72, P, stageP, true, st));
+    e = cudaMemcpyAsync(U_host, stageU, fb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P_host, stageP, fb, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) {
+        set_error("%s: D2H copy: %s", fn, cudaGetErrorString(e));
+        return QCD_ECUDA;
+    }
+    return QCD_OK;
+}
+
+}  // extern "C"

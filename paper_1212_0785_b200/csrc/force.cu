@@ -1,0 +1,195 @@
+// force.cu — Wilson gauge force (O7; "force term calculation", "projection of
+// fields"), optionally fused with the momentum update P += eps*F (fewer site loops).
+//
+// One thread per site of the subset, all four directions.  A thread block owns the
+// sites of a compact 4-D tile so that the 44 neighbour links a site needs are shared through L1.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "qcd_internal.h"
+#include "site.cuh"
+#include "su3.cuh"
+
+namespace qcd {
+
+// thread -> site of the block's tile
+__device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile) {
+    int j = threadIdx.x;
+    int par = tile.par0;
+    if (tile.npar == 2) {
+        par = j >= tile.tsp ? 1 : 0;
+        j -= par * tile.tsp;
+    }
+    const int hx = tile.T[0] >> 1;
+    int r = j / hx;
+    const int jx = j - r * hx;
+    const int jy = r % tile.T[1];
+    r /= tile.T[1];
+    const int jz = r % tile.T[2];
+    const int jt = r / tile.T[2];
+    int b = blockIdx.x;
+    const int bx = b % tile.nt[0];
+    b /= tile.nt[0];
+    const int by = b % tile.nt[1];
+    b /= tile.nt[1];
+    const int bz = b % tile.nt[2];
+    const int bt = b / tile.nt[2];
+    Site st;
+    st.par = par;
+    st.c[1] = by * tile.T[1] + jy;
+    st.c[2] = bz * tile.T[2] + jz;
+    st.c[3] = bt * tile.T[3] + jt;
+    st.c[0] = bx * tile.T[0] + 2 * jx + ((st.c[1] + st.c[2] + st.c[3] + par) & 1);
+    st.s = st.c[0] + lat.L[0] * (st.c[1] + lat.L[1] * (st.c[2] + lat.L[2] * st.c[3]));
+    return st;
+}
+
+// F_mu(x) for mu = 0..3 at the thread's site; FUSED: out = P, P += eps F; else out = F.
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
+                                                    const T eps, const pair_t<T> *__restrict__ U,
+                                                    pair_t<T> *__restrict__ out) {
+    const Site st = tile_site(lat, tile);
+    const int V = lat.V;
+    const int par = st.par;
+    const int cb = cb_of(lat, st.s, par);
+    int df[4], db[4];
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+        df[d] = dfwd(lat, st, d);
+        db[d] = dbwd(lat, st, d);
+    }
+
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu++) {
+        const int dfm = mu == 0 ? df[0] : mu == 1 ? df[1] : mu == 2 ? df[2] : df[3];
+        const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
+        M3<T> A;
+        zero(A);
+#pragma unroll
+        for (int k = 1; k < 4; k++) {
+            const int nu = (mu + k) & 3;
+            const int dfn = nu == 0 ? df[0] : nu == 1 ? df[1] : nu == 2 ? df[2] : df[3];
+            const int dbn = nu == 0 ? db[0] : nu == 1 ? db[1] : nu == 2 ? db[2] : db[3];
+            const int cb_pn = cb_of(lat, st.s + dfn, par ^ 1);      // x + nu
+            const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
+            const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
+            M3<T> X, Y, Z;
+            // up staple: U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+            load_link(X, U, V, nu, cb_pm);
+            load_link(Y, U, V, mu, cb_pn);
+            mul<false, true, false>(Z, X, Y);
+            load_link(X, U, V, nu, cb);
+            mul<false, true, true>(A, Z, X);
+            // down staple: U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu)
+            load_link(X, U, V, nu, cb_pmmn);
+            load_link(Y, U, V, mu, cb_mn);
+            mul<true, true, false>(Z, X, Y);
+            load_link(X, U, V, nu, cb_mn);
+            mul<false, false, true>(A, Z, X);
+        }
+        M3<T> Um, W;
+        load_link(Um, U, V, mu, cb);
+        mul<false, false, false>(W, Um, A);
+        M3<T> F;
+        project_force(F, W, c);
+        if (FUSED) {
+            M3<T> P;
+            load_link_rw(P, out, V, mu, cb);
+#pragma unroll
+            for (int e = 0; e < 9; e++) {
+                P.re[e] = fma_(eps, F.re[e], P.re[e]);
+                P.im[e] = fma_(eps, F.im[e], P.im[e]);
+            }
+            store_link(P, out, V, mu, cb);
+        } else {
+            store_link(F, out, V, mu, cb);
+        }
+    }
+}
+
+// ---- host side: tile choice -------------------------------------------------------------------
+
+// all divisors of n (even ones only if `even`)
+static int divisors(int n, bool even, int *out) {
+    int k = 0;
+    for (int d = 1; d <= n; d++)
+        if (n % d == 0 && (!even || (d & 1) == 0)) out[k++] = d;
+    return k;
+}
+
+// Pick tile extents dividing L with T0 even and `threads` = T0/2*T1*T2*T3*npar as close to the target
+// as possible (never above 256), preferring a long x extent (coalescing: T0/2 consecutive sites are
+// contiguous in memory) and then the smallest surface (L1 reuse of neighbour links).
+// QCD_TILE="tx,ty,tz,tt" overrides for block-shape sweeps (the paper's N_t tuning).
+static TileP choose_tile(const LatP &lat, int subset) {
+    TileP tp;
+    tp.npar = subset == QCD_ALL ? 2 : 1;
+    tp.par0 = subset == QCD_ODD ? 1 : 0;
+    int best[4] = {2, 1, 1, 1};
+    const char *env = getenv("QCD_TILE");
+    int e[4];
+    bool have = false;
+    if (env && sscanf(env, "%d,%d,%d,%d", &e[0], &e[1], &e[2], &e[3]) == 4) {
+        have = true;
+        for (int d = 0; d < 4; d++)
+            if (e[d] < 1 || lat.L[d] % e[d]) have = false;
+        if (e[0] & 1) have = false;
+        if (have && (long)(e[0] / 2) * e[1] * e[2] * e[3] * tp.npar > 256) have = false;
+        if (have) memcpy(best, e, sizeof e);
+    }
+    if (!have) {
+        const int target = 256;
+        int dv[4][128], nd[4];
+        for (int d = 0; d < 4; d++) nd[d] = divisors(lat.L[d], d == 0, dv[d]);
+        double best_score = -1e300;
+        for (int a = 0; a < nd[0]; a++)
+            for (int b = 0; b < nd[1]; b++)
+                for (int cc = 0; cc < nd[2]; cc++)
+                    for (int d = 0; d < nd[3]; d++) {
+                        const int t[4] = {dv[0][a], dv[1][b], dv[2][cc], dv[3][d]};
+                        const long threads = (long)(t[0] / 2) * t[1] * t[2] * t[3] * tp.npar;
+                        if (threads > target) continue;
+                        const double vol = (double)t[0] * t[1] * t[2] * t[3];
+                        double surf = 0;
+                        for (int k = 0; k < 4; k++) surf += vol / t[k];
+                        // more threads first; then x extent up to 16 (128-byte rows in fp64); then compactness
+                        const double score = threads * 1e6 + (t[0] >= 16 ? 16 : t[0]) * 1e3 - surf / vol * 100.0;
+                        if (score > best_score) {
+                            best_score = score;
+                            memcpy(best, t, sizeof t);
+                        }
+                    }
+    }
+    for (int d = 0; d < 4; d++) {
+        tp.T[d] = best[d];
+        tp.nt[d] = lat.L[d] / best[d];
+    }
+    tp.tsp = (tp.T[0] / 2) * tp.T[1] * tp.T[2] * tp.T[3];
+    return tp;
+}
+
+template <typename T>
+static int launch_force_t(const qcd_lattice *lat, int subset, double beta, double eps, const void *U, void *out,
+                          bool fused, cudaStream_t st) {
+    const TileP tp = choose_tile(lat->p, subset);
+    const int threads = tp.tsp * tp.npar;
+    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+    const T c = (T)(beta / 12.0);
+    if (fused)
+        force_kernel<T, true><<<blocks, threads, 0, st>>>(lat->p, tp, c, (T)eps, (const pair_t<T> *)U,
+                                                           (pair_t<T> *)out);
+    else
+        force_kernel<T, false><<<blocks, threads, 0, st>>>(lat->p, tp, c, (T)eps, (const pair_t<T> *)U,
+                                                            (pair_t<T> *)out);
+    return check_launch(fused ? "force_mom_update" : "gauge_force");
+}
+
+int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
+                       void *out, bool fused_mom, cudaStream_t st) {
+    return prec == QCD_F64 ? launch_force_t<double>(lat, subset, beta, eps, U, out, fused_mom, st)
+                           : launch_force_t<float>(lat, subset, beta, eps, U, out, fused_mom, st);
+}
+
+}  // namespace qcd

@@ -1,0 +1,76 @@
+// qcd_internal.h — host/device shared declarations of libqcdmd (not part of the public ABI).
+//
+// Device layout (include/qcd.h): a matrix field is an array of 36*V complex pairs; entry
+// (mu, e=3*row+col) of checkerboard site cb sits at pair index (mu*9+e)*V + cb.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/qcd.h"
+
+namespace qcd {
+
+// Lattice geometry handed to kernels by value.
+struct LatP {
+    int L[4];       // extents
+    int stride[4];  // lexicographic strides 1, Lx, Lx*Ly, Lx*Ly*Lz
+    int V;          // sites
+    int Vh;         // V/2 sites per parity
+};
+
+// 4-D tile handled by one thread block of the stencil kernels (force).  The block owns the sites
+// of `npar` parities of the tile; T[0] is even so every x-row has T[0]/2 sites of each parity.
+struct TileP {
+    int T[4];   // tile extents (divide L)
+    int nt[4];  // tiles per direction
+    int tsp;    // sites per parity per tile = T0/2*T1*T2*T3
+    int npar;   // parities per block: 2 (subset ALL) or 1
+    int par0;   // parity handled when npar == 1
+};
+
+// Reduction geometry (fixed, independent of any tuning, so results are run-to-run identical).
+constexpr int RED_THREADS = 256;   // threads per reduction block
+constexpr int RED_CHUNK = 1024;    // sites per first-pass block
+constexpr int RED_GENERIC_CHUNKS = 256;  // first-pass blocks per subset on the subset_id path
+constexpr int MAX_NSUB = 4096;
+constexpr int MAX_SUM_NCOMP = 64;
+
+}  // namespace qcd
+
+struct qcd_lattice {
+    qcd::LatP p;
+    int red_chunks_per_seg;  // first-pass blocks per (timeslice, parity) segment
+    int red_nseg;            // 2*Lt segments
+    size_t workspace_doubles;
+};
+
+namespace qcd {
+
+void set_error(const char *fmt, ...);
+int check_launch(const char *what);
+
+// kernel launchers, one per translation unit; prec already validated. All return QCD_OK/QCD_ECUDA.
+int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
+                       void *out, bool fused_mom, cudaStream_t st);
+int launch_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P,
+                      cudaStream_t st);
+int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,
+                       int mode /*0 exp, 1 exp+reunit, 2 reunit only*/, cudaStream_t st);
+int launch_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *P,
+                       cudaStream_t st);
+int launch_hot_start(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, cudaStream_t st);
+int launch_perturb(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, cudaStream_t st);
+int launch_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, const uint32_t *site,
+                      const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, cudaStream_t st);
+int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                     double *ws, cudaStream_t st);
+int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, const void *field, double *out,
+               double *ws, cudaStream_t st);
+int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
+                     const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st);
+int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex, void *soa, bool unpack,
+                cudaStream_t st);
+int launch_get_map(const qcd_lattice *lat, int which, int32_t *out, cudaStream_t st);
+
+}  // namespace qcd

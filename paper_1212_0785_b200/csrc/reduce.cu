@@ -1,0 +1,222 @@
+// reduce.cu — plaquette (O6) and the global / per-subset sums (O12; "sum, sumMulti").
+//
+// Deterministic two-pass reductions: the lattice is cut into (timeslice, parity) segments, each a
+// contiguous range of checkerboard indices, and every segment into fixed chunks of RED_CHUNK sites.
+// Pass 1: one block per chunk, fixed per-thread order, fixed shuffle/shared tree -> one partial.
+// Pass 2: one block per result sums the partials in a fixed order.  The geometry depends only on
+// the lattice, never on tuning, so results are bit-identical from run to run.
+#include "qcd_internal.h"
+#include "site.cuh"
+#include "su3.cuh"
+
+namespace qcd {
+
+// fixed-order block sum; result valid in thread 0
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double warp_part[RED_THREADS / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) warp_part[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < RED_THREADS / 32; k++) r += warp_part[k];
+    }
+    __syncthreads();
+    return r;
+}
+
+// ---- per-site values -----------------------------------------------------------------------
+
+// sum_{mu<nu} Re tr P_mu_nu(x), P_mu_nu(x) = [U_mu(x) U_nu(x+mu)] [U_nu(x) U_mu(x+nu)]^dagger
+template <typename T>
+__device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T> *__restrict__ U, int cb) {
+    const Site st = site_of_cb(lat, cb);
+    const int V = lat.V;
+    int cbf[4];
+#pragma unroll
+    for (int d = 0; d < 4; d++) cbf[d] = cb_of(lat, st.s + dfwd(lat, st, d), st.par ^ 1);
+    T acc = T(0);
+#pragma unroll
+    for (int mu = 0; mu < 3; mu++) {
+        M3<T> Um;
+        load_link(Um, U, V, mu, cb);
+#pragma unroll
+        for (int nu = mu + 1; nu < 4; nu++) {
+            M3<T> A, X, Y;
+            load_link(A, U, V, nu, cbf[mu]);
+            mul<false, false, false>(X, Um, A);
+            M3<T> B;
+            load_link(A, U, V, nu, cb);
+            load_link(B, U, V, mu, cbf[nu]);
+            mul<false, false, false>(Y, A, B);
+            acc += retr_mul_dag(X, Y);
+        }
+    }
+    return (double)acc;
+}
+
+template <typename T>
+__device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int V, const T *__restrict__ f, int cb) {
+    if (kind == QCD_SUM_SCALAR) return (double)__ldg(f + (size_t)comp * V + cb);
+    double acc = 0.0;
+    if (kind == QCD_SUM_NORM2) {
+        const pair_t<T> *p = (const pair_t<T> *)f;
+        for (int k = 0; k < ncomp / 2; k++) {
+            const pair_t<T> v = __ldg(p + (size_t)k * V + cb);
+            acc = fma((double)v.x, (double)v.x, acc);
+            acc = fma((double)v.y, (double)v.y, acc);
+        }
+    } else {
+        const pair_t<T> *p = (const pair_t<T> *)f;
+        for (int m = 0; m < ncomp / 18; m++) {
+            acc += (double)__ldg(p + (size_t)(m * 9 + 0) * V + cb).x;
+            acc += (double)__ldg(p + (size_t)(m * 9 + 4) * V + cb).x;
+            acc += (double)__ldg(p + (size_t)(m * 9 + 8) * V + cb).x;
+        }
+    }
+    return acc;
+}
+
+// ---- pass 1 --------------------------------------------------------------------------------
+
+// grid (chunks_per_seg, nseg, ncomp_out); kind < 0: plaquette.
+// partial[(comp*nseg + seg)*cps + chunk], seg = 2*t + parity
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, const int kind, const int ncomp,
+                                                            const void *__restrict__ field, double *__restrict__ partial) {
+    const int cps = gridDim.x, nseg = gridDim.y;
+    const int seg = blockIdx.y, comp = blockIdx.z;
+    const int Vsh = lat.Vh / lat.L[3];
+    const int seg_begin = (seg & 1) * lat.Vh + (seg >> 1) * Vsh;
+    double acc = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < RED_CHUNK / RED_THREADS; k++) {
+        const int i = blockIdx.x * RED_CHUNK + k * RED_THREADS + threadIdx.x;
+        if (i < Vsh) {
+            const int cb = seg_begin + i;
+            acc += kind < 0 ? site_plaquette<T>(lat, (const pair_t<T> *)field, cb)
+                            : site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb);
+        }
+    }
+    const double r = block_sum(acc);
+    if (threadIdx.x == 0) partial[((size_t)comp * nseg + seg) * cps + blockIdx.x] = r;
+}
+
+// subset_id path: grid (RED_GENERIC_CHUNKS, nsub, ncomp_out); partial[(comp*nsub + k)*RED_GENERIC_CHUNKS + chunk]
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) reduce_pass1_ids(const LatP lat, const int kind, const int ncomp,
+                                                                const void *__restrict__ field,
+                                                                const int32_t *__restrict__ ids,
+                                                                double *__restrict__ partial) {
+    const int k = blockIdx.y, comp = blockIdx.z, nsub = gridDim.y;
+    const int csize = (lat.V + RED_GENERIC_CHUNKS - 1) / RED_GENERIC_CHUNKS;
+    const int begin = blockIdx.x * csize;
+    const int end = min(begin + csize, lat.V);
+    double acc = 0.0;
+    for (int cb = begin + threadIdx.x; cb < end; cb += RED_THREADS)
+        if (__ldg(ids + cb) == k) acc += site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb);
+    const double r = block_sum(acc);
+    if (threadIdx.x == 0) partial[((size_t)comp * nsub + k) * RED_GENERIC_CHUNKS + blockIdx.x] = r;
+}
+
+// ---- pass 2 --------------------------------------------------------------------------------
+
+// out[blockIdx.x * out_stride + comp] = scale * sum of `count` partials starting at
+// partial[(comp*ngroups + blockIdx.x) * count], taking every `step`-th group member if step > 1 ...
+// Written generally: group g = blockIdx.x covers partial indices base(g) + i*stride_i, i < count.
+__global__ void __launch_bounds__(RED_THREADS) reduce_pass2(const double *__restrict__ partial, const int ngroups,
+                                                            const int count, const double scale,
+                                                            double *__restrict__ out, const int out_stride) {
+    const int g = blockIdx.x, comp = blockIdx.y;
+    const double *p = partial + ((size_t)comp * ngroups + g) * count;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < count; i += RED_THREADS) acc += p[i];
+    const double r = block_sum(acc);
+    if (threadIdx.x == 0) out[(size_t)g * out_stride + comp] = scale * r;
+}
+
+// global sum over the segments of one parity set: segments seg with (seg&1)==par if par<2, all if par==2
+__global__ void __launch_bounds__(RED_THREADS) reduce_pass2_global(const double *__restrict__ partial, const int nseg,
+                                                                   const int cps, const int par, const double scale,
+                                                                   double *__restrict__ out) {
+    const int comp = blockIdx.x;
+    const double *p = partial + (size_t)comp * nseg * cps;
+    double acc = 0.0;
+    if (par == 2) {
+        for (int i = threadIdx.x; i < nseg * cps; i += RED_THREADS) acc += p[i];
+    } else {
+        const int n = (nseg / 2) * cps;
+        for (int i = threadIdx.x; i < n; i += RED_THREADS) {
+            const int t = i / cps, c = i - t * cps;
+            acc += p[(size_t)(2 * t + par) * cps + c];
+        }
+    }
+    const double r = block_sum(acc);
+    if (threadIdx.x == 0) out[comp] = scale * r;
+}
+
+// ---- launchers -----------------------------------------------------------------------------
+
+template <typename T>
+static int plaquette_t(const qcd_lattice *lat, const void *U, double *out_avg, double *out_per_t, double *ws,
+                       cudaStream_t st) {
+    const LatP &p = lat->p;
+    const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
+    reduce_pass1<T><<<dim3(cps, nseg, 1), RED_THREADS, 0, st>>>(p, -1, 72, U, ws);
+    const int Lt = p.L[3];
+    const double Vs = (double)(p.V / Lt);
+    if (out_per_t)  // segments 2t, 2t+1 are adjacent: one group of 2*cps partials per timeslice
+        reduce_pass2<<<dim3(Lt, 1), RED_THREADS, 0, st>>>(ws, Lt, 2 * cps, 1.0 / (18.0 * Vs), out_per_t, 1);
+    reduce_pass2_global<<<1, RED_THREADS, 0, st>>>(ws, nseg, cps, 2, 1.0 / (18.0 * (double)p.V), out_avg);
+    return check_launch("plaquette");
+}
+
+int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t, double *ws,
+                     cudaStream_t st) {
+    return prec == QCD_F64 ? plaquette_t<double>(lat, U, out_avg, out_per_t, ws, st)
+                           : plaquette_t<float>(lat, U, out_avg, out_per_t, ws, st);
+}
+
+template <typename T>
+static int sum_t(const qcd_lattice *lat, int subset, int kind, int ncomp, const void *field, double *out, double *ws,
+                 cudaStream_t st) {
+    const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
+    const int nout = kind == QCD_SUM_SCALAR ? ncomp : 1;
+    reduce_pass1<T><<<dim3(cps, nseg, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field, ws);
+    const int par = subset == QCD_ALL ? 2 : subset == QCD_EVEN ? 0 : 1;
+    reduce_pass2_global<<<nout, RED_THREADS, 0, st>>>(ws, nseg, cps, par, 1.0, out);
+    return check_launch("sum");
+}
+
+int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, const void *field, double *out,
+               double *ws, cudaStream_t st) {
+    return prec == QCD_F64 ? sum_t<double>(lat, subset, kind, ncomp, field, out, ws, st)
+                           : sum_t<float>(lat, subset, kind, ncomp, field, out, ws, st);
+}
+
+template <typename T>
+static int sum_multi_t(const qcd_lattice *lat, int kind, int ncomp, const void *field, const int32_t *ids, int nsub,
+                       double *out, double *ws, cudaStream_t st) {
+    const int nout = kind == QCD_SUM_SCALAR ? ncomp : 1;
+    if (!ids) {
+        const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
+        reduce_pass1<T><<<dim3(cps, nseg, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field, ws);
+        reduce_pass2<<<dim3(nsub, nout), RED_THREADS, 0, st>>>(ws, nsub, 2 * cps, 1.0, out, nout);
+    } else {
+        reduce_pass1_ids<T><<<dim3(RED_GENERIC_CHUNKS, nsub, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field,
+                                                                                          ids, ws);
+        reduce_pass2<<<dim3(nsub, nout), RED_THREADS, 0, st>>>(ws, nsub, RED_GENERIC_CHUNKS, 1.0, out, nout);
+    }
+    return check_launch("sum_multi");
+}
+
+int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
+                     const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st) {
+    return prec == QCD_F64 ? sum_multi_t<double>(lat, kind, ncomp, field, subset_id, nsub, out, ws, st)
+                           : sum_multi_t<float>(lat, kind, ncomp, field, subset_id, nsub, out, ws, st);
+}
+
+}  // namespace qcd

@@ -1,0 +1,276 @@
+// su3.cuh — 3x3 complex algebra in registers, templated on the real type (double / float).
+// Everything is fully unrolled with compile-time indices so matrices live in registers.
+#pragma once
+
+#include <cuda_runtime.h>
+
+namespace qcd {
+
+template <typename T> struct Pair;
+template <> struct Pair<double> { using type = double2; };
+template <> struct Pair<float> { using type = float2; };
+template <typename T> using pair_t = typename Pair<T>::type;
+
+template <typename T>
+struct M3 {
+    T re[9];
+    T im[9];
+};
+
+template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
+template <> __device__ __forceinline__ double fma_<double>(double a, double b, double c) { return fma(a, b, c); }
+template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
+
+template <typename T> __device__ __forceinline__ T rsqrt_(T a);
+template <> __device__ __forceinline__ double rsqrt_<double>(double a) { return 1.0 / sqrt(a); }
+template <> __device__ __forceinline__ float rsqrt_<float>(float a) { return 1.0f / sqrtf(a); }
+
+// ---- global memory access: entry (mu,e) of site cb at pair index (mu*9+e)*V + cb
+
+template <typename T>
+__device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
+    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        pair_t<T> v = __ldg(p + (size_t)e * V);
+        m.re[e] = v.x;
+        m.im[e] = v.y;
+    }
+}
+
+// same, through the normal (coherent) path: for fields the kernel also writes
+template <typename T>
+__device__ __forceinline__ void load_link_rw(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {
+    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        pair_t<T> v = p[(size_t)e * V];
+        m.re[e] = v.x;
+        m.im[e] = v.y;
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ void store_link(const M3<T> &m, pair_t<T> *f, int V, int mu, int cb) {
+    pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        pair_t<T> v;
+        v.x = m.re[e];
+        v.y = m.im[e];
+        p[(size_t)e * V] = v;
+    }
+}
+
+// ---- products.  DA / DB: take the dagger of that operand.  ACC: C += ... instead of C = ...
+
+template <bool DA, bool DB, bool ACC, typename T>
+__device__ __forceinline__ void mul(M3<T> &C, const M3<T> &A, const M3<T> &B) {
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            T cr = ACC ? C.re[3 * i + j] : T(0);
+            T ci = ACC ? C.im[3 * i + j] : T(0);
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                const int ia = DA ? 3 * k + i : 3 * i + k;
+                const int ib = DB ? 3 * j + k : 3 * k + j;
+                const T ar = A.re[ia], ai = DA ? -A.im[ia] : A.im[ia];
+                const T br = B.re[ib], bi = DB ? -B.im[ib] : B.im[ib];
+                cr = fma_(ar, br, cr);
+                cr = fma_(-ai, bi, cr);
+                ci = fma_(ar, bi, ci);
+                ci = fma_(ai, br, ci);
+            }
+            C.re[3 * i + j] = cr;
+            C.im[3 * i + j] = ci;
+        }
+}
+
+// Re tr (A B^dagger) = sum_ij Re(A_ij conj(B_ij))
+template <typename T>
+__device__ __forceinline__ T retr_mul_dag(const M3<T> &A, const M3<T> &B) {
+    T acc = T(0);
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        acc = fma_(A.re[e], B.re[e], acc);
+        acc = fma_(A.im[e], B.im[e], acc);
+    }
+    return acc;
+}
+
+template <typename T>
+__device__ __forceinline__ void zero(M3<T> &A) {
+#pragma unroll
+    for (int e = 0; e < 9; e++) A.re[e] = A.im[e] = T(0);
+}
+
+// ---- projection (O7): F = (i c)[(W - W^dag) - (1/3) tr(W - W^dag)], c = beta/12.
+// W - W^dag =: X is anti-Hermitian: X_ii = 2i Im W_ii, X_ij = W_ij - conj(W_ji).
+// i*X is Hermitian; F_ii = -2c (Im W_ii - mean Im W_kk), F_ij = i c (W_ij - conj(W_ji)).
+template <typename T>
+__device__ __forceinline__ void project_force(M3<T> &F, const M3<T> &W, T c) {
+    const T m = (W.im[0] + W.im[4] + W.im[8]) * T(1.0 / 3.0);
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        F.re[4 * i] = T(-2) * c * (W.im[4 * i] - m);
+        F.im[4 * i] = T(0);
+    }
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = i + 1; j < 3; j++) {
+            const T xr = W.re[3 * i + j] - W.re[3 * j + i];
+            const T xi = W.im[3 * i + j] + W.im[3 * j + i];
+            // i c (xr + i xi) = -c xi + i c xr
+            F.re[3 * i + j] = -c * xi;
+            F.im[3 * i + j] = c * xr;
+            F.re[3 * j + i] = -c * xi;
+            F.im[3 * j + i] = -c * xr;
+        }
+}
+
+// ---- reunitarisation (O9): row Gram-Schmidt, third row = conj(r0 x r1)
+template <typename T>
+__device__ __forceinline__ void reunit(M3<T> &M) {
+    T n0 = T(0);
+#pragma unroll
+    for (int j = 0; j < 3; j++) n0 = fma_(M.re[j], M.re[j], fma_(M.im[j], M.im[j], n0));
+    T s = rsqrt_(n0);
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        M.re[j] *= s;
+        M.im[j] *= s;
+    }
+    // d = r0^dag . r1
+    T dr = T(0), di = T(0);
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        dr = fma_(M.re[j], M.re[3 + j], dr);
+        dr = fma_(M.im[j], M.im[3 + j], dr);
+        di = fma_(M.re[j], M.im[3 + j], di);
+        di = fma_(-M.im[j], M.re[3 + j], di);
+    }
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        // r1 -= d r0
+        M.re[3 + j] = fma_(-dr, M.re[j], fma_(di, M.im[j], M.re[3 + j]));
+        M.im[3 + j] = fma_(-dr, M.im[j], fma_(-di, M.re[j], M.im[3 + j]));
+    }
+    T n1 = T(0);
+#pragma unroll
+    for (int j = 0; j < 3; j++) n1 = fma_(M.re[3 + j], M.re[3 + j], fma_(M.im[3 + j], M.im[3 + j], n1));
+    s = rsqrt_(n1);
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        M.re[3 + j] *= s;
+        M.im[3 + j] *= s;
+    }
+    // r2 = conj(r0 x r1): (a x b)_0 = a1 b2 - a2 b1, ...
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const int a = (j + 1) % 3, b = (j + 2) % 3;
+        const T pr = M.re[a] * M.re[3 + b] - M.im[a] * M.im[3 + b] - (M.re[b] * M.re[3 + a] - M.im[b] * M.im[3 + a]);
+        const T pi = M.re[a] * M.im[3 + b] + M.im[a] * M.re[3 + b] - (M.re[b] * M.im[3 + a] + M.im[b] * M.re[3 + a]);
+        M.re[6 + j] = pr;
+        M.im[6 + j] = -pi;
+    }
+}
+
+// ---- exp(iQ) for Hermitian traceless Q (O8), Cayley-Hamilton route.
+// Q^3 = c1 Q + c0 with c1 = (1/2) tr Q^2, c0 = det Q = (1/3) tr Q^3 (both real), hence
+// (iQ)^k / k! = a_k + b_k Q + c_k Q^2 with (a,b,c)_{k+1} = (i/(k+1)) (c0 c_k, a_k + c1 c_k, b_k).
+// Q is first scaled by 2^-n so that ||Q||_F <= 1 (series terms decay from the start: no
+// cancellation), the result squared n times.  NT = number of series terms kept.
+template <typename T> struct ExpTerms;
+template <> struct ExpTerms<double> { static constexpr int max_terms = 22; static constexpr double tol = 1e-18; };
+template <> struct ExpTerms<float> { static constexpr int max_terms = 13; static constexpr float tol = 1e-9f; };
+
+template <typename T>
+__device__ __forceinline__ void expi_herm(M3<T> &E, const M3<T> &Qin) {
+    T n2 = T(0);
+#pragma unroll
+    for (int e = 0; e < 9; e++) n2 = fma_(Qin.re[e], Qin.re[e], fma_(Qin.im[e], Qin.im[e], n2));
+    int nsq = 0;
+    T scale = T(1);
+    while (n2 * scale * scale > T(1)) {
+        scale *= T(0.5);
+        nsq++;
+    }
+    M3<T> Q;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        Q.re[e] = Qin.re[e] * scale;
+        Q.im[e] = Qin.im[e] * scale;
+    }
+    n2 *= scale * scale;
+    M3<T> Q2;
+    mul<false, false, false>(Q2, Q, Q);
+    const T c1 = T(0.5) * n2;
+    // c0 = (1/3) Re tr(Q Q2) = (1/3) sum_ij Re(Q_ij Q2_ji)
+    T c0 = T(0);
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            c0 = fma_(Q.re[3 * i + j], Q2.re[3 * j + i], c0);
+            c0 = fma_(-Q.im[3 * i + j], Q2.im[3 * j + i], c0);
+        }
+    c0 *= T(1.0 / 3.0);
+    // series
+    T ar = T(1), ai = T(0), br = T(0), bi = T(0), cr = T(0), ci = T(0);
+    T f0r = T(1), f0i = T(0), f1r = T(0), f1i = T(0), f2r = T(0), f2i = T(0);
+    // bound on the k-th term: x^k/k! with x = ||Q||_F <= 1
+    T x = sqrt(n2), bound = T(1);
+    for (int k = 1; k <= ExpTerms<T>::max_terms; k++) {
+        const T inv = T(1) / T(k);
+        // (a,b,c) <- (i/k) (c0 c, a + c1 c, b);  i (x + i y) = -y + i x
+        const T tar = c0 * cr, tai = c0 * ci;
+        const T tbr = fma_(c1, cr, ar), tbi = fma_(c1, ci, ai);
+        const T tcr = br, tci = bi;
+        ar = -tai * inv; ai = tar * inv;
+        br = -tbi * inv; bi = tbr * inv;
+        cr = -tci * inv; ci = tcr * inv;
+        f0r += ar; f0i += ai;
+        f1r += br; f1i += bi;
+        f2r += cr; f2i += ci;
+        bound *= x * inv;
+        if (bound < ExpTerms<T>::tol) break;
+    }
+    // E = f0 + f1 Q + f2 Q2
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        T er = fma_(f1r, Q.re[e], fma_(-f1i, Q.im[e], fma_(f2r, Q2.re[e], -f2i * Q2.im[e])));
+        T ei = fma_(f1r, Q.im[e], fma_(f1i, Q.re[e], fma_(f2r, Q2.im[e], f2i * Q2.re[e])));
+        if (e == 0 || e == 4 || e == 8) {
+            er += f0r;
+            ei += f0i;
+        }
+        E.re[e] = er;
+        E.im[e] = ei;
+    }
+    for (int k = 0; k < nsq; k++) {
+        M3<T> S;
+        mul<false, false, false>(S, E, E);
+        E = S;
+    }
+}
+
+// Q = sum_a q_a T_a (O2), T_a = Gell-Mann / 2
+template <typename T>
+__device__ __forceinline__ void herm_from_coeffs(M3<T> &Q, const double q[8]) {
+    const double is3 = 0.57735026918962576451;  // 1/sqrt(3)
+    Q.re[0] = T(q[2] / 2 + q[7] * is3 / 2);
+    Q.re[4] = T(-q[2] / 2 + q[7] * is3 / 2);
+    Q.re[8] = T(-q[7] * is3);
+    Q.im[0] = Q.im[4] = Q.im[8] = T(0);
+    Q.re[1] = T(q[0] / 2); Q.im[1] = T(-q[1] / 2);
+    Q.re[2] = T(q[3] / 2); Q.im[2] = T(-q[4] / 2);
+    Q.re[5] = T(q[5] / 2); Q.im[5] = T(-q[6] / 2);
+    Q.re[3] = Q.re[1]; Q.im[3] = -Q.im[1];
+    Q.re[6] = Q.re[2]; Q.im[6] = -Q.im[2];
+    Q.re[7] = Q.re[5]; Q.im[7] = -Q.im[5];
+}
+
+}  // namespace qcd

@@ -1,0 +1,529 @@
+"""GPU parity: the CUDA path (through the C ABI of include/qcd.h) against the CPU oracle, element by
+element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; norm per DESIGN.md R15): fields max|gpu-ref| / max|ref| <= 1e-12 in
+fp64 and 2e-5 in fp32; scalars |d|/|ref|; integer maps and RNG words bit-exact.  fp32 runs feed the
+fp64 oracle the fp32-rounded inputs (R14).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from tests import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-5}
+
+
+@pytest.fixture(scope="module")
+def qcd():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1212_0785_b200 import binding
+    return binding
+
+
+def tdtype(prec):
+    import torch
+    return torch.float64 if prec == "f64" else torch.float32
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def round_to(prec, a):
+    """inputs as the GPU sees them: fp32-rounded for the fp32 path"""
+    if prec == "f64":
+        return a
+    return a.astype(np.complex64).astype(np.complex128) if np.iscomplexobj(a) else a.astype(np.float32).astype(np.float64)
+
+
+def dev(qcd, lat, a, prec):
+    return qcd.field_to_device(lat, a, tdtype(prec))
+
+
+def host(qcd, lat, t):
+    return qcd.field_to_host(lat, t)
+
+
+def sync():
+    import torch
+    torch.cuda.synchronize()
+
+
+DIMS_SMALL = [(2, 2, 2, 2), (4, 4, 4, 4), (6, 4, 2, 8), (4, 10, 6, 2), (8, 8, 8, 16)]
+
+
+# ------------------------------------------------------------------ integer work: bit-exact
+
+@pytest.mark.parametrize("dims", DIMS_SMALL + [(16, 16, 16, 32), (12, 6, 10, 4)])
+def test_maps_bit_exact(qcd, orc, dims):
+    import torch
+    lat = qcd.Lattice(dims)
+    out = torch.empty(lat.V, dtype=torch.int32, device="cuda")
+    for which in range(12):
+        out.fill_(-1)
+        qcd.qcd_get_map(lat, which, out)
+        assert np.array_equal(out.cpu().numpy(), orc.map(dims, which)), which
+
+
+def test_rng_words_and_uniforms_bit_exact(qcd, orc):
+    import torch
+    n = 4096
+    rng = np.random.default_rng(7)
+    site = rng.integers(0, 2 ** 31 - 1, n, dtype=np.int64).astype(np.uint32)
+    site[:4] = [0, 1, 0xFFFFFFFF, 10616831]
+    mu_j = rng.integers(0, 64, n).astype(np.uint32)
+    seed, stream_id, purpose = 0x1212078500000003, 5, 1
+    d_site = torch.from_numpy(site.view(np.int32)).cuda()
+    d_muj = torch.from_numpy(mu_j.view(np.int32)).cuda()
+    words = torch.empty(4 * n, dtype=torch.int32, device="cuda")
+    uni = torch.empty(2 * n, dtype=torch.float64, device="cuda")
+    gau = torch.empty(2 * n, dtype=torch.float64, device="cuda")
+    qcd.qcd_rng_blocks(seed, stream_id, purpose, d_site, d_muj, words, uni, gau)
+    w = words.cpu().numpy().view(np.uint32).reshape(n, 4)
+    u = uni.cpu().numpy().reshape(n, 2)
+    g = gau.cpu().numpy().reshape(n, 2)
+    for i in range(n):
+        rw, ru, rg = orc.rng_block(seed, int(site[i]), int(mu_j[i]) // 16, int(mu_j[i]) % 16, stream_id, purpose)
+        assert list(w[i]) == rw
+        assert u[i, 0] == ru[0] and u[i, 1] == ru[1]  # exact dyadic uniforms
+        assert np.abs(g[i] - rg).max() < 1e-14 * max(1.0, np.abs(rg).max())
+    # empty request is a no-op
+    e = torch.empty(0, dtype=torch.int32, device="cuda")
+    qcd.qcd_rng_blocks(seed, 0, 0, e, e)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_pack_unpack_layout(qcd, orc, prec):
+    import torch
+    dims = (4, 6, 2, 4)
+    lat = qcd.Lattice(dims)
+    V = lat.V
+    A = round_to(prec, inputs.random_matrix_field(3, V))
+    d = dev(qcd, lat, A, prec)
+    assert np.array_equal(host(qcd, lat, d), A)  # round trip is exact
+    # documented layout: pair (mu*9+e) of site cb at pair index (mu*9+e)*V + cb
+    raw = d.cpu().numpy().astype(np.float64)  # [36][V][2]
+    cb = orc.map(dims, O.MAP_CB_OF_LEX)
+    ref = np.empty((36, V, 2))
+    flat = A.reshape(V, 36)
+    ref[:, cb, 0] = flat.real.T
+    ref[:, cb, 1] = flat.imag.T
+    assert np.array_equal(raw, ref)
+    # real-field layout [comp][cb]
+    R = round_to(prec, inputs.random_real_field(4, V, 3))
+    src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
+    dst = lat.new_real_field(3, tdtype(prec))
+    qcd.qcd_pack(lat, 3, src, dst)
+    got = dst.cpu().numpy().astype(np.float64)
+    assert np.array_equal(got[:, cb], R.T)
+
+
+# ------------------------------------------------------------------ generators
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 8)])
+def test_mom_refresh_and_hot_start(qcd, orc_omp, prec, dims):
+    lat = qcd.Lattice(dims)
+    seed = inputs.config_seed(3)
+    tol = TOL[prec] if prec == "f64" else 2e-7  # fp32: fp64 Gaussians rounded once
+    P = lat.new_matrix_field(tdtype(prec))
+    qcd.qcd_mom_refresh(lat, P, seed, stream_id=2)
+    ref = orc_omp.mom_refresh(dims, seed, stream_id=2)
+    assert rel(host(qcd, lat, P), ref) < tol
+    par = orc_omp.map(dims, O.MAP_PARITY)
+    for subset, keep in ((qcd.EVEN, 1), (qcd.ODD, 0)):
+        P.fill_(7.0)
+        qcd.qcd_mom_refresh(lat, P, seed, stream_id=2, subset=subset)
+        got = host(qcd, lat, P)
+        assert np.all(got[par == keep] == 7.0 + 7.0j)  # other parity untouched, bit-identical
+        assert rel(got[par != keep], ref[par != keep]) < tol
+    U = lat.new_matrix_field(tdtype(prec))
+    for sigma in (0.2, 0.5, 3.0):
+        qcd.qcd_hot_start(lat, U, seed, sigma)
+        assert rel(host(qcd, lat, U), orc_omp.hot_start(dims, seed, sigma)) < tol * (10 if sigma > 1 else 1)
+
+
+# ------------------------------------------------------------------ plaquette, sums
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", DIMS_SMALL + [(16, 16, 16, 32)])
+def test_plaquette(qcd, orc_omp, prec, dims):
+    import torch
+    lat = qcd.Lattice(dims)
+    U = round_to(prec, orc_omp.hot_start(dims, inputs.config_seed(3), 0.5))
+    dU = dev(qcd, lat, U, prec)
+    ws = lat.new_workspace()
+    avg = torch.zeros(1, dtype=torch.float64, device="cuda")
+    per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
+    qcd.qcd_plaquette(lat, dU, avg, per_t, ws)
+    ravg, rper_t = orc_omp.plaquette(dims, U)
+    tol = TOL[prec]
+    assert abs(avg.item() - ravg) / abs(ravg) < tol
+    assert rel(per_t.cpu().numpy(), rper_t) < tol
+    assert abs(per_t.mean().item() - avg.item()) < 1e-14
+    # deterministic: bit-identical on a second run, and without the per-timeslice output
+    avg2 = torch.zeros(1, dtype=torch.float64, device="cuda")
+    qcd.qcd_plaquette(lat, dU, avg2, None, ws)
+    assert avg2.item() == avg.item()
+    # generic (non-unitary) matrices exercise every entry of the products
+    G = round_to(prec, inputs.random_matrix_field(5, lat.V) * 0.7)
+    qcd.qcd_plaquette(lat, dev(qcd, lat, G, prec), avg, per_t, ws)
+    gavg, gper_t = orc_omp.plaquette(dims, G)
+    scale = np.abs(gper_t).max()
+    assert np.abs(per_t.cpu().numpy() - gper_t).max() / scale < tol * 50  # sums of O(1) terms of both signs
+    assert abs(avg.item() - gavg) / scale < tol * 50
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 6, 2, 8), (16, 16, 16, 32)])
+def test_sum_and_sum_multi(qcd, orc, prec, dims):
+    import torch
+    lat = qcd.Lattice(dims)
+    V, Lt = lat.V, dims[3]
+    ws = lat.new_workspace()
+    tol = 1e-12 if prec == "f64" else 1e-6  # inputs identical (rounded), accumulation always fp64
+    cb = orc.map(dims, O.MAP_CB_OF_LEX)
+    # matrix kinds on a momentum-like field
+    M = round_to(prec, inputs.random_matrix_field(11, V))
+    dM = dev(qcd, lat, M, prec)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for kind, okind in ((qcd.SUM_NORM2, O.SUM_NORM2), (qcd.SUM_RETR, O.SUM_RETR)):
+        scale = np.sum(np.abs(M) ** 2) if kind == qcd.SUM_NORM2 else np.abs(np.trace(M, axis1=-2, axis2=-1).real).sum()
+        for subset in (qcd.ALL, qcd.EVEN, qcd.ODD):
+            qcd.qcd_sum(lat, kind, 72, dM, out, ws, subset=subset)
+            assert abs(out.item() - orc.sum(dims, okind, M, subset=subset)[0]) / scale < tol, (kind, subset)
+        outt = torch.zeros(Lt, dtype=torch.float64, device="cuda")
+        qcd.qcd_sum_multi(lat, kind, 72, dM, None, Lt, outt, ws)
+        assert np.abs(outt.cpu().numpy() - orc.sum_multi(dims, okind, M)).max() / scale < tol
+        nsub = 7
+        ids = inputs.random_subset_ids(5, V, nsub)
+        ids[::11] = -1  # sites in no subset
+        ids_cb = np.empty_like(ids)
+        ids_cb[cb] = ids
+        outs = torch.zeros(nsub, dtype=torch.float64, device="cuda")
+        qcd.qcd_sum_multi(lat, kind, 72, dM, torch.from_numpy(ids_cb).cuda(), nsub, outs, ws)
+        assert np.abs(outs.cpu().numpy() - orc.sum_multi(dims, okind, M, subset_id=ids, nsub=nsub)).max() / scale < tol
+    # scalar kind, 3 components, closed forms included
+    R = inputs.random_real_field(13, V, 3)
+    R[:, 1] = orc.map(dims, O.MAP_TSLICE)
+    R[:, 2] = 1 - 2 * orc.map(dims, O.MAP_PARITY)
+    R = round_to(prec, R)
+    dR = lat.new_real_field(3, tdtype(prec))
+    qcd.qcd_pack(lat, 3, torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1), dR)
+    out3 = torch.zeros(3, dtype=torch.float64, device="cuda")
+    for subset in (qcd.ALL, qcd.EVEN, qcd.ODD):
+        qcd.qcd_sum(lat, qcd.SUM_SCALAR, 3, dR, out3, ws, subset=subset)
+        ref = orc.sum(dims, O.SUM_SCALAR, R, subset=subset)
+        got = out3.cpu().numpy()
+        assert abs(got[0] - ref[0]) < tol * np.abs(R[:, 0]).sum()
+        assert got[1] == ref[1] and got[2] == ref[2]  # integer-valued sums are exact
+    assert out3[2].item() == -V / 2
+    outm = torch.zeros(Lt * 3, dtype=torch.float64, device="cuda")
+    qcd.qcd_sum_multi(lat, qcd.SUM_SCALAR, 3, dR, None, Lt, outm, ws)
+    refm = orc.sum_multi(dims, O.SUM_SCALAR, R)
+    got = outm.cpu().numpy().reshape(Lt, 3)
+    assert np.abs(got[:, 0] - refm[:, 0]).max() < tol * np.abs(R[:, 0]).sum()
+    assert np.array_equal(got[:, 1:], refm[:, 1:])
+
+
+# ------------------------------------------------------------------ force, momentum update
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", DIMS_SMALL + [(16, 16, 16, 32), (12, 6, 10, 4)])
+def test_gauge_force_all_subsets(qcd, orc_omp, prec, dims):
+    lat = qcd.Lattice(dims)
+    beta = 5.8
+    U = round_to(prec, orc_omp.hot_start(dims, inputs.config_seed(3), 0.5))
+    dU = dev(qcd, lat, U, prec)
+    ref = orc_omp.gauge_force(dims, beta, U)
+    par = orc_omp.map(dims, O.MAP_PARITY)
+    F = lat.new_matrix_field(tdtype(prec))
+    qcd.qcd_gauge_force(lat, dU, F, beta)
+    got = host(qcd, lat, F)
+    assert rel(got, ref) < TOL[prec]
+    assert np.abs(got - np.conj(np.swapaxes(got, -1, -2))).max() == 0  # exactly Hermitian by construction
+    for subset, keep in ((qcd.EVEN, 1), (qcd.ODD, 0)):
+        F.fill_(3.0)
+        qcd.qcd_gauge_force(lat, dU, F, beta, subset=subset)
+        got = host(qcd, lat, F)
+        assert np.all(got[par == keep] == 3.0 + 3.0j)
+        assert rel(got[par != keep], ref[par != keep]) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_gauge_force_generic_matrices(qcd, orc, prec):
+    """O7 is a formula on arbitrary 3x3 matrices; non-unitary input catches any dagger/order slip"""
+    dims = (4, 6, 4, 2)
+    lat = qcd.Lattice(dims)
+    U = round_to(prec, inputs.random_matrix_field(17, lat.V) * 0.6)
+    F = lat.new_matrix_field(tdtype(prec))
+    qcd.qcd_gauge_force(lat, dev(qcd, lat, U, prec), F, 6.1)
+    assert rel(host(qcd, lat, F), orc.gauge_force(dims, 6.1, U)) < TOL[prec] * 5
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 32)])
+def test_mom_update_and_fused_force_mom_update(qcd, orc_omp, prec, dims):
+    lat = qcd.Lattice(dims)
+    beta, eps = 5.8, 0.05
+    U = round_to(prec, orc_omp.hot_start(dims, inputs.config_seed(3), 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, inputs.config_seed(3)))
+    Fr = orc_omp.gauge_force(dims, beta, U)
+    par = orc_omp.map(dims, O.MAP_PARITY)
+    dU = dev(qcd, lat, U, prec)
+    for subset, osub in ((qcd.ALL, O.ALL), (qcd.EVEN, O.EVEN), (qcd.ODD, O.ODD)):
+        # unfused: F from the oracle (rounded), P += eps F
+        Fin = round_to(prec, Fr)
+        dP = dev(qcd, lat, P, prec)
+        qcd.qcd_mom_update(lat, dev(qcd, lat, Fin, prec), dP, eps, subset=subset)
+        ref = orc_omp.mom_update(dims, eps, Fin, P, subset=osub)
+        got = host(qcd, lat, dP)
+        assert rel(got, ref) < (1e-15 if prec == "f64" else 2e-7)  # one rounding (FMA vs mul+add)
+        # fused
+        dP = dev(qcd, lat, P, prec)
+        qcd.qcd_force_mom_update(lat, dU, dP, beta, eps, subset=subset)
+        ref = orc_omp.mom_update(dims, eps, Fr, P, subset=osub)
+        got = host(qcd, lat, dP)
+        assert rel(got, ref) < TOL[prec]
+        if subset != qcd.ALL:
+            keep = 1 if subset == qcd.EVEN else 0
+            assert np.array_equal(got[par == keep], P[par == keep])
+
+
+# ------------------------------------------------------------------ link update, reunitarisation
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (6, 4, 2, 8), (16, 16, 16, 32)])
+def test_link_update_and_reunit(qcd, orc_omp, prec, dims):
+    lat = qcd.Lattice(dims)
+    eps = 0.05
+    seed = inputs.config_seed(3)
+    U = round_to(prec, orc_omp.hot_start(dims, seed, 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, seed))
+    par = orc_omp.map(dims, O.MAP_PARITY)
+    dP = dev(qcd, lat, P, prec)
+    for reunit in (False, True):
+        for subset, osub in ((qcd.ALL, O.ALL), (qcd.EVEN, O.EVEN), (qcd.ODD, O.ODD)):
+            dU = dev(qcd, lat, U, prec)
+            qcd.qcd_link_update(lat, dP, dU, eps, reunit=reunit, subset=subset)
+            got = host(qcd, lat, dU)
+            ref = orc_omp.link_update(dims, eps, P, U, reunit=reunit, subset=osub)
+            assert rel(got, ref) < TOL[prec], (reunit, subset)
+            if subset != qcd.ALL:
+                keep = 1 if subset == qcd.EVEN else 0
+                assert np.array_equal(got[par == keep], U[par == keep])
+    # large steps: exp(i eps P) for norms far beyond the series radius (scaling and squaring path)
+    for big in (1.0, 7.0, 40.0):
+        dU = dev(qcd, lat, U, prec)
+        qcd.qcd_link_update(lat, dP, dU, big, reunit=False)
+        ref = orc_omp.link_update(dims, big, P, U)
+        assert rel(host(qcd, lat, dU), ref) < TOL[prec] * max(1.0, big), big
+    # reunitarisation of links pushed off SU(3) by sigma = 1e-3 noise (config 3), GPU noise vs oracle noise
+    dU = dev(qcd, lat, U, prec)
+    qcd.qcd_perturb(lat, dU, seed + 1, 1e-3)
+    Up = round_to(prec, orc_omp.perturb(dims, seed + 1, 1e-3, U))
+    assert rel(host(qcd, lat, dU), Up) < (1e-14 if prec == "f64" else 2e-7)
+    for subset, osub in ((qcd.ALL, O.ALL), (qcd.EVEN, O.EVEN), (qcd.ODD, O.ODD)):
+        dU = dev(qcd, lat, Up, prec)
+        qcd.qcd_reunit(lat, dU, subset=subset)
+        got = host(qcd, lat, dU)
+        assert rel(got, orc_omp.reunit(dims, Up, subset=osub)) < TOL[prec]
+        if subset != qcd.ALL:
+            keep = 1 if subset == qcd.EVEN else 0
+            assert np.array_equal(got[par == keep], Up[par == keep])
+    if prec == "f64":
+        got = host(qcd, lat, dU)[par == 1]
+        assert np.abs(got @ np.conj(np.swapaxes(got, -1, -2)) - np.eye(3)).max() < 1e-14
+
+
+def test_expi_degenerate_and_zero_momenta(qcd, orc):
+    """exp of Q = 0 and of Q with degenerate eigenvalues (T8 direction), through qcd_link_update"""
+    dims = (2, 2, 2, 2)
+    lat = qcd.Lattice(dims)
+    V = lat.V
+    U = orc.hot_start(dims, 3, 0.5)
+    P = np.zeros((V, 4, 3, 3), dtype=np.complex128)
+    P[1::2, :] = np.diag([1.0, 1.0, -2.0]) / np.sqrt(12.0)
+    P[2, 1] = np.diag([0.3, -0.3, 0.0])
+    for eps in (0.1, 3.0):
+        dU = dev(qcd, lat, U, "f64")
+        qcd.qcd_link_update(lat, dev(qcd, lat, P, "f64"), dU, eps)
+        got = host(qcd, lat, dU)
+        assert rel(got, orc.link_update(dims, eps, P, U)) < 1e-12
+        assert np.array_equal(got[0], U[0])  # P = 0 -> exp = 1 exactly -> U unchanged
+
+
+# ------------------------------------------------------------------ configs 1 and 2: trajectories
+
+def gpu_H(qcd, lat, dU, dP, beta, ws):
+    import torch
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, dP, out[0:1], ws)
+    qcd.qcd_plaquette(lat, dU, out[1:2], None, ws)
+    K, plaq = out.cpu().numpy()
+    return K, beta * 6 * lat.V * (1 - plaq), plaq
+
+
+def test_config1_one_leapfrog_step(qcd, orc):
+    c = inputs.CONFIGS[1]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    seed = inputs.config_seed(1)
+    lat = qcd.Lattice(dims)
+    ws = lat.new_workspace()
+    U0 = orc.hot_start(dims, seed, c["sigma"])
+    P0 = orc.mom_refresh(dims, seed)
+    # the GPU generates its own start from the same (seed, counter) definition
+    dU = lat.new_matrix_field()
+    dP = lat.new_matrix_field()
+    qcd.qcd_hot_start(lat, dU, seed, c["sigma"])
+    qcd.qcd_mom_refresh(lat, dP, seed)
+    assert rel(host(qcd, lat, dU), U0) < 1e-12 and rel(host(qcd, lat, dP), P0) < 1e-12
+    K0, S0, plaq0 = gpu_H(qcd, lat, dU, dP, beta, ws)
+    rK0, rS0 = orc.hamiltonian(dims, beta, U0, P0)
+    assert abs(K0 - rK0) / rK0 < 1e-12 and abs(S0 - rS0) / rS0 < 1e-12
+    assert abs(plaq0 - orc.plaquette(dims, U0)[0]) < 1e-12
+    qcd.qcd_leapfrog(lat, dU, dP, beta, eps, 1)
+    U1, P1 = orc.leapfrog(dims, beta, eps, 1, U0, P0)
+    assert rel(host(qcd, lat, dU), U1) < 1e-12 and rel(host(qcd, lat, dP), P1) < 1e-12
+    K1, S1, plaq1 = gpu_H(qcd, lat, dU, dP, beta, ws)
+    rK1, rS1 = orc.hamiltonian(dims, beta, U1, P1)
+    dH, rdH = (K1 + S1) - (K0 + S0), (rK1 + rS1) - (rK0 + rS0)
+    assert abs(dH - rdH) <= 1e-12 * abs(rK0 + rS0)  # DESIGN.md R15: dH against |H|
+    assert abs(plaq1 - orc.plaquette(dims, U1)[0]) < 1e-12 and abs(K1 - rK1) / rK1 < 1e-12
+
+
+def test_config2_trajectory_parity_each_step_and_reversibility(qcd, orc_omp):
+    c = inputs.CONFIGS[2]
+    dims, beta, eps, n = c["dims"], c["beta"], c["eps"], c["nsteps"]
+    seed = inputs.config_seed(2)
+    lat = qcd.Lattice(dims)
+    ws = lat.new_workspace()
+    U = orc_omp.hot_start(dims, seed, c["sigma"])
+    P = orc_omp.mom_refresh(dims, seed)
+    U0, P0 = U.copy(), P.copy()
+    dU, dP = dev(qcd, lat, U, "f64"), dev(qcd, lat, P, "f64")
+    K0, S0, _ = gpu_H(qcd, lat, dU, dP, beta, ws)
+    # leapfrog as its steps (O11): P += eps/2 F; n x { U update+reunit; P += eps F (eps/2 last) }
+    qcd.qcd_force_mom_update(lat, dU, dP, beta, eps / 2)
+    P = orc_omp.mom_update(dims, eps / 2, orc_omp.gauge_force(dims, beta, U), P)
+    for k in range(n):
+        e = eps / 2 if k == n - 1 else eps
+        qcd.qcd_link_update(lat, dP, dU, eps, reunit=True)
+        qcd.qcd_force_mom_update(lat, dU, dP, beta, e)
+        U = orc_omp.link_update(dims, eps, P, U, reunit=True)
+        P = orc_omp.mom_update(dims, e, orc_omp.gauge_force(dims, beta, U), P)
+        assert rel(host(qcd, lat, dU), U) < 1e-12, k
+        assert rel(host(qcd, lat, dP), P) < 1e-12, k
+    K1, S1, plaq1 = gpu_H(qcd, lat, dU, dP, beta, ws)
+    rK0, rS0 = orc_omp.hamiltonian(dims, beta, U0, P0)
+    rK1, rS1 = orc_omp.hamiltonian(dims, beta, U, P)
+    assert abs(((K1 + S1) - (K0 + S0)) - ((rK1 + rS1) - (rK0 + rS0))) <= 1e-12 * abs(rK0 + rS0)
+    assert abs(plaq1 - orc_omp.plaquette(dims, U)[0]) < 1e-12
+    # reversed trajectory through the single-call driver returns to the start
+    dP.mul_(-1.0)
+    qcd.qcd_leapfrog(lat, dU, dP, beta, eps, n)
+    dP.mul_(-1.0)
+    assert rel(host(qcd, lat, dU), U0) < 1e-12
+    assert rel(host(qcd, lat, dP), P0) < 1e-12
+
+
+def test_fp32_trajectory_tracks_fp64_oracle(qcd, orc_omp):
+    c = inputs.CONFIGS[2]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    seed = inputs.config_seed(2)
+    lat = qcd.Lattice(dims)
+    U = round_to("f32", orc_omp.hot_start(dims, seed, c["sigma"]))
+    P = round_to("f32", orc_omp.mom_refresh(dims, seed))
+    dU, dP = dev(qcd, lat, U, "f32"), dev(qcd, lat, P, "f32")
+    qcd.qcd_leapfrog(lat, dU, dP, beta, eps, 10)
+    U1, P1 = orc_omp.leapfrog(dims, beta, eps, 10, U, P)
+    assert rel(host(qcd, lat, dU), U1) < 2e-5 and rel(host(qcd, lat, dP), P1) < 2e-5
+
+
+# ------------------------------------------------------------------ full sizes, in bench.py's launch configuration
+
+def sample_sites(dims, n, seed):
+    """lexicographic sites: corners and faces of the lattice (periodic wrap) plus random interior ones"""
+    Lx, Ly, Lz, Lt = dims
+    rng = np.random.default_rng(seed)
+    pts = []
+    for x in (0, 1, Lx - 1):
+        for y in (0, Ly - 1):
+            for z in (0, Lz - 1):
+                for t in (0, 1, Lt - 1):
+                    pts.append(x + Lx * (y + Ly * (z + Lz * t)))
+    pts += list(rng.integers(0, Lx * Ly * Lz * Lt, n - len(pts)))
+    return np.unique(np.array(pts, dtype=np.int32))
+
+
+@pytest.mark.parametrize("cfg,prec", [(4, "f64"), (5, "f32")])
+def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec):
+    """BASELINE configs 4 (32^3x64 fp64, the headline) and 5 (48^3x96): the fused MD step exactly as
+    bench.py launches it (qcd_md_step, subset ALL), checked at sampled sites the oracle computes one
+    by one, plus properties that hold at any size."""
+    import torch
+    c = inputs.CONFIGS[cfg]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    seed = inputs.config_seed(cfg)
+    lat = qcd.Lattice(dims)
+    dt = tdtype(prec)
+    dU, dP = lat.new_matrix_field(dt), lat.new_matrix_field(dt)
+    qcd.qcd_hot_start(lat, dU, seed, c["sigma"])
+    qcd.qcd_mom_refresh(lat, dP, seed)
+    # the oracle builds the same start from the (seed, counter) definition, never from the GPU
+    U0 = orc_omp.hot_start(dims, seed, c["sigma"])
+    sites = sample_sites(dims, 600, 1)
+    cbmap = orc_omp.map(dims, O.MAP_CB_OF_LEX)
+    cbs = torch.from_numpy(cbmap[sites].astype(np.int64)).cuda()
+
+    def gather(field):  # device field [36][V][2] -> complex [n,4,3,3] at the sampled sites
+        g = field[:, cbs, :].to(torch.float64).cpu().numpy()
+        return (g[..., 0] + 1j * g[..., 1]).T.reshape(len(sites), 4, 3, 3)
+
+    tolgen = 1e-12 if prec == "f64" else 2e-7
+    assert rel(gather(dU), U0[sites]) < tolgen
+    if prec == "f32":  # the fp32 path starts from rounded links: give the oracle the same (in place, chunked)
+        flat = U0.reshape(-1).view(np.float64)
+        for i in range(0, flat.size, 1 << 26):
+            flat[i:i + (1 << 26)] = flat[i:i + (1 << 26)].astype(np.float32)
+    # momenta at the sampled sites from the oracle's generator blocks (the RNG is keyed on the site)
+    Psites = np.empty((len(sites), 4, 3, 3), dtype=np.complex128)
+    for i, s_ in enumerate(sites):
+        for mu in range(4):
+            q = np.concatenate([orc_omp.rng_block(seed, int(s_), mu, j, 0, 1)[2] for j in range(4)])
+            Psites[i, mu] = orc_omp.herm_from_coeffs(q)
+    assert rel(gather(dP), Psites) < tolgen
+    Psites = round_to(prec, Psites)
+    ws = lat.new_workspace()
+    plaq = torch.zeros(1, dtype=torch.float64, device="cuda")
+    per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
+    qcd.qcd_plaquette(lat, dU, plaq, per_t, ws)
+    rplaq, rper_t = orc_omp.plaquette(dims, U0)
+    assert abs(plaq.item() - rplaq) / rplaq < TOL[prec]
+    assert rel(per_t.cpu().numpy(), rper_t) < TOL[prec]
+    # one fused MD step
+    qcd.qcd_md_step(lat, dU, dP, beta, eps, eps)
+    Fs = orc_omp.gauge_force_sites(dims, beta, U0, sites)
+    P1 = Psites + eps * Fs
+    assert rel(gather(dP), P1) < TOL[prec]
+    # link update is site-local: run the oracle on the sampled sites laid out as a small lattice
+    n = len(sites) // 16 * 16
+    sub = (2, 2, 2, n // 8)
+    U1 = orc_omp.link_update(sub, eps, np.ascontiguousarray(P1[:n]), np.ascontiguousarray(U0[sites][:n]), reunit=True)
+    gU = gather(dU)
+    assert rel(gU[:n], U1) < TOL[prec]
+    # any-size properties: links stay in SU(3), momenta stay Hermitian traceless
+    utol = 1e-14 if prec == "f64" else 1e-6
+    assert np.abs(gU @ np.conj(np.swapaxes(gU, -1, -2)) - np.eye(3)).max() < utol
+    assert np.abs(np.linalg.det(gU) - 1).max() < utol
+    gP = gather(dP)
+    assert np.abs(gP - np.conj(np.swapaxes(gP, -1, -2))).max() < utol * 10
+    assert np.abs(np.trace(gP, axis1=-2, axis2=-1)).max() < utol * 10
+    # kinetic energy of the updated momenta: K/(16 V) stays near 1 for this small step
+    K = torch.zeros(1, dtype=torch.float64, device="cuda")
+    qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, dP, K, ws)
+    assert abs(K.item() / (16 * lat.V) - 1) < 0.01

@@ -487,3 +487,11 @@ def test_serial_and_openmp_builds_agree_bitwise(orc, orc_omp):
     assert np.array_equal(Ua, Ub) and np.array_equal(Pa, Pb)
     assert orc.plaquette(dims, Ua)[0] == orc_omp.plaquette(dims, Ub)[0]
     assert orc.num_threads() == 1
+
+
+def test_force_at_listed_sites_is_the_full_force(orc):
+    dims = (4, 4, 2, 4)
+    U = orc.hot_start(dims, 3, 0.5)
+    F = orc.gauge_force(dims, 5.5, U)
+    sites = np.array([0, 5, 127, 17, 5], dtype=np.int32)
+    assert np.array_equal(orc.gauge_force_sites(dims, 5.5, U, sites), F[sites])
