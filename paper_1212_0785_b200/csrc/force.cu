@@ -14,8 +14,7 @@
 namespace qcd {
 
 // thread -> site of the block's tile
-__device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile) {
-    int j = threadIdx.x;
+__device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, int j) {
     int par = tile.par0;
     if (tile.npar == 2) {
         par = j >= tile.tsp ? 1 : 0;
@@ -50,7 +49,7 @@ template <typename T, bool FUSED>
 __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out) {
-    const Site st = tile_site(lat, tile);
+    const Site st = tile_site(lat, tile, threadIdx.x);
     const int V = lat.V;
     const int par = st.par;
     const int cb = cb_of(lat, st.s, par);
@@ -109,6 +108,68 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
     }
 }
 
+// Variant "link": one thread per (site, mu).  The block owns the same 4-D tile; thread j < nsite handles
+// mu = 0, the next nsite threads mu = 1, ... (mu is warp-uniform when nsite is a multiple of 32).  A
+// quarter of the per-thread state of the per-site variant: more warps in flight per SM.
+template <typename T, bool FUSED, int NT>
+__global__ void __launch_bounds__(NT) force_link_kernel(const LatP lat, const TileP tile, const T c, const T eps,
+                                                       const pair_t<T> *__restrict__ U,
+                                                       pair_t<T> *__restrict__ out) {
+    const int nsite = tile.tsp * tile.npar;
+    const int mu = threadIdx.x / nsite;
+    const Site st = tile_site(lat, tile, threadIdx.x - mu * nsite);
+    const int V = lat.V;
+    const int par = st.par;
+    const int cb = cb_of(lat, st.s, par);
+    int df[4], db[4];
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+        df[d] = dfwd(lat, st, d);
+        db[d] = dbwd(lat, st, d);
+    }
+    const int dfm = mu == 0 ? df[0] : mu == 1 ? df[1] : mu == 2 ? df[2] : df[3];
+    const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
+    M3<T> A;
+    zero(A);
+#pragma unroll 1
+    for (int k = 1; k < 4; k++) {
+        const int nu = (mu + k) & 3;
+        const int dfn = nu == 0 ? df[0] : nu == 1 ? df[1] : nu == 2 ? df[2] : df[3];
+        const int dbn = nu == 0 ? db[0] : nu == 1 ? db[1] : nu == 2 ? db[2] : db[3];
+        const int cb_pn = cb_of(lat, st.s + dfn, par ^ 1);      // x + nu
+        const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
+        const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
+        M3<T> X, Y, Z;
+        load_link(X, U, V, nu, cb_pm);
+        load_link(Y, U, V, mu, cb_pn);
+        mul<false, true, false>(Z, X, Y);
+        load_link(X, U, V, nu, cb);
+        mul<false, true, true>(A, Z, X);
+        load_link(X, U, V, nu, cb_pmmn);
+        load_link(Y, U, V, mu, cb_mn);
+        mul<true, true, false>(Z, X, Y);
+        load_link(X, U, V, nu, cb_mn);
+        mul<false, false, true>(A, Z, X);
+    }
+    M3<T> Um, W;
+    load_link(Um, U, V, mu, cb);
+    mul<false, false, false>(W, Um, A);
+    M3<T> F;
+    project_force(F, W, c);
+    if (FUSED) {
+        M3<T> P;
+        load_link_rw(P, out, V, mu, cb);
+#pragma unroll
+        for (int e = 0; e < 9; e++) {
+            P.re[e] = fma_(eps, F.re[e], P.re[e]);
+            P.im[e] = fma_(eps, F.im[e], P.im[e]);
+        }
+        store_link(P, out, V, mu, cb);
+    } else {
+        store_link(F, out, V, mu, cb);
+    }
+}
+
 // ---- host side: tile choice -------------------------------------------------------------------
 
 // all divisors of n (even ones only if `even`)
@@ -120,10 +181,10 @@ static int divisors(int n, bool even, int *out) {
 }
 
 // Pick tile extents dividing L with T0 even and `threads` = T0/2*T1*T2*T3*npar as close to the target
-// as possible (never above 256), preferring a long x extent (coalescing: T0/2 consecutive sites are
+// as possible (never above it), preferring a long x extent (coalescing: T0/2 consecutive sites are
 // contiguous in memory) and then the smallest surface (L1 reuse of neighbour links).
 // QCD_TILE="tx,ty,tz,tt" overrides for block-shape sweeps (the paper's N_t tuning).
-static TileP choose_tile(const LatP &lat, int subset) {
+static TileP choose_tile(const LatP &lat, int subset, int target) {
     TileP tp;
     tp.npar = subset == QCD_ALL ? 2 : 1;
     tp.par0 = subset == QCD_ODD ? 1 : 0;
@@ -136,11 +197,10 @@ static TileP choose_tile(const LatP &lat, int subset) {
         for (int d = 0; d < 4; d++)
             if (e[d] < 1 || lat.L[d] % e[d]) have = false;
         if (e[0] & 1) have = false;
-        if (have && (long)(e[0] / 2) * e[1] * e[2] * e[3] * tp.npar > 256) have = false;
+        if (have && (long)(e[0] / 2) * e[1] * e[2] * e[3] * tp.npar > target) have = false;
         if (have) memcpy(best, e, sizeof e);
     }
     if (!have) {
-        const int target = 256;
         int dv[4][128], nd[4];
         for (int d = 0; d < 4; d++) nd[d] = divisors(lat.L[d], d == 0, dv[d]);
         double best_score = -1e300;
@@ -170,19 +230,35 @@ static TileP choose_tile(const LatP &lat, int subset) {
     return tp;
 }
 
+// QCD_FORCE_VARIANT selects the kernel for block-shape / mapping sweeps (the paper's N_t tuning,
+// PAPER.md:57): "site" = one thread per site (256 threads), "link" = one thread per (site, mu) with
+// QCD_FORCE_THREADS in {256, 512} threads per block.
+template <typename T, bool FUSED>
+static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const pair_t<T> *U, pair_t<T> *out,
+                           cudaStream_t st) {
+    const char *v = getenv("QCD_FORCE_VARIANT");
+    const bool site = v && !strcmp(v, "site");
+    if (site) {
+        const TileP tp = choose_tile(lat->p, subset, 256);
+        const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+        force_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        return;
+    }
+    const char *t = getenv("QCD_FORCE_THREADS");
+    const int nt = t ? atoi(t) : 512;
+    const TileP tp = choose_tile(lat->p, subset, nt == 256 ? 64 : 128);
+    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+    const int threads = 4 * tp.tsp * tp.npar;
+    if (nt == 256) force_link_kernel<T, FUSED, 256><<<blocks, threads, 0, st>>>(lat->p, tp, c, eps, U, out);
+    else force_link_kernel<T, FUSED, 512><<<blocks, threads, 0, st>>>(lat->p, tp, c, eps, U, out);
+}
+
 template <typename T>
 static int launch_force_t(const qcd_lattice *lat, int subset, double beta, double eps, const void *U, void *out,
                           bool fused, cudaStream_t st) {
-    const TileP tp = choose_tile(lat->p, subset);
-    const int threads = tp.tsp * tp.npar;
-    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
     const T c = (T)(beta / 12.0);
-    if (fused)
-        force_kernel<T, true><<<blocks, threads, 0, st>>>(lat->p, tp, c, (T)eps, (const pair_t<T> *)U,
-                                                           (pair_t<T> *)out);
-    else
-        force_kernel<T, false><<<blocks, threads, 0, st>>>(lat->p, tp, c, (T)eps, (const pair_t<T> *)U,
-                                                            (pair_t<T> *)out);
+    if (fused) launch_force_v<T, true>(lat, subset, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
+    else launch_force_v<T, false>(lat, subset, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
     return check_launch(fused ? "force_mom_update" : "gauge_force");
 }
 
