@@ -45,7 +45,7 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
 }
 
 // F_mu(x) for mu = 0..3 at the thread's site; FUSED: out = P, P += eps F; else out = F.
-template <typename T, bool FUSED>
+template <typename T, bool FUSED, int PMODE>
 __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out) {
@@ -60,11 +60,19 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         db[d] = dbwd(lat, st, d);
     }
 
+    if (FUSED && PMODE >= 2) {  // start pulling this thread's momenta towards the SM before the staple work
+#pragma unroll 4
+        for (int e = 0; e < 36; e++) {
+            if (PMODE == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(out + (size_t)e * V + cb));
+            else asm volatile("prefetch.global.L1 [%0];" ::"l"(out + (size_t)e * V + cb));
+        }
+    }
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
         const int dfm = mu == 0 ? df[0] : mu == 1 ? df[1] : mu == 2 ? df[2] : df[3];
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
-        M3<T> A;
+        M3<T> A, Pm;
+        if (FUSED && PMODE == 1) load_link_rw(Pm, out, V, mu, cb);
         zero(A);
 #pragma unroll
         for (int k = 1; k < 4; k++) {
@@ -95,7 +103,8 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         project_force(F, W, c);
         if (FUSED) {
             M3<T> P;
-            load_link_rw(P, out, V, mu, cb);
+            if (PMODE == 1) P = Pm;
+            else load_link_rw(P, out, V, mu, cb);
 #pragma unroll
             for (int e = 0; e < 9; e++) {
                 P.re[e] = fma_(eps, F.re[e], P.re[e]);
@@ -237,11 +246,16 @@ template <typename T, bool FUSED>
 static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const pair_t<T> *U, pair_t<T> *out,
                            cudaStream_t st) {
     const char *v = getenv("QCD_FORCE_VARIANT");
-    const bool site = v && !strcmp(v, "site");
+    const bool site = !v || strcmp(v, "link");
     if (site) {
         const TileP tp = choose_tile(lat->p, subset, 256);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
-        force_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        const char *pm = getenv("QCD_PMODE");
+        const int pmode = pm ? atoi(pm) : 0;
+        if (pmode == 1) force_kernel<T, FUSED, 1><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        else if (pmode == 2) force_kernel<T, FUSED, 2><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        else if (pmode == 3) force_kernel<T, FUSED, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        else force_kernel<T, FUSED, 0><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
         return;
     }
     const char *t = getenv("QCD_FORCE_THREADS");
@@ -262,8 +276,19 @@ static int launch_force_t(const qcd_lattice *lat, int subset, double beta, doubl
     return check_launch(fused ? "force_mom_update" : "gauge_force");
 }
 
+// Kernel choice.  Default: the plain staple kernels of this file (the definition, valid for arbitrary 3x3
+// matrices and for subsets).  QCD_FORCE_VARIANT = site | link | tile | plaq selects a variant for the
+// block-shape / mapping sweeps (the paper's N_t auto-tuning); tile (force_tile.cu) and plaq
+// (force_plaq.cu, needs unitary links) exist for subset ALL only.  DESIGN.md section 6 has the measurements.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
                        void *out, bool fused_mom, cudaStream_t st) {
+    const char *v = getenv("QCD_FORCE_VARIANT");
+    if (subset == QCD_ALL && v && !strcmp(v, "plaq"))
+        return launch_gauge_force_plaq(lat, prec, beta, eps, U, out, fused_mom, st);
+    if (subset == QCD_ALL && v && !strcmp(v, "tile")) {
+        const int rc = launch_gauge_force_tile(lat, prec, beta, eps, U, out, fused_mom, st);
+        if (rc >= 0) return rc;
+    }
     return prec == QCD_F64 ? launch_force_t<double>(lat, subset, beta, eps, U, out, fused_mom, st)
                            : launch_force_t<float>(lat, subset, beta, eps, U, out, fused_mom, st);
 }

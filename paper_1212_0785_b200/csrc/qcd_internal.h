@@ -53,6 +53,12 @@ int check_launch(const char *what);
 // kernel launchers, one per translation unit; prec already validated. All return QCD_OK/QCD_ECUDA.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
                        void *out, bool fused_mom, cudaStream_t st);
+// plaquette-sharing force kernel (force_plaq.cu): subset ALL, unitary links
+int launch_gauge_force_plaq(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *out,
+                            bool fused_mom, cudaStream_t st);
+// staple kernel with the tile's own links staged in shared memory (force_tile.cu): subset ALL; -1 = not applicable
+int launch_gauge_force_tile(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *out,
+                            bool fused_mom, cudaStream_t st);
 int launch_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P,
                       cudaStream_t st);
 int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,

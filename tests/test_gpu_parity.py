@@ -266,6 +266,36 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("link", None), ("tile", None),
+                                          ("tile", "8,2,2,4"), ("tile", "4,4,4,4"), ("plaq", None),
+                                          ("plaq", "8,4,2,2"), ("plaq", "4,2,4,2")])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 4), (16, 8, 8, 16)])
+def test_force_kernel_variants(qcd, orc_omp, monkeypatch, prec, variant, tile, dims):
+    """every selectable force kernel (QCD_FORCE_VARIANT, QCD_TILE: the block-shape sweep knobs) against the
+    oracle, fused and unfused, on SU(3) links (the plaq variant needs unitary links), over several tiles
+    and with tiles that span a whole extent (periodic wrap inside the tile)"""
+    monkeypatch.setenv("QCD_FORCE_VARIANT", variant)
+    if tile:
+        if any(d % t for d, t in zip(dims, map(int, tile.split(",")))):
+            pytest.skip("tile does not divide the lattice")
+        monkeypatch.setenv("QCD_TILE", tile)
+    else:
+        monkeypatch.delenv("QCD_TILE", raising=False)
+    lat = qcd.Lattice(dims)
+    beta, eps = 6.0, 0.07
+    U = round_to(prec, orc_omp.hot_start(dims, inputs.config_seed(2), 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, inputs.config_seed(2)))
+    Fr = orc_omp.gauge_force(dims, beta, U)
+    dU = dev(qcd, lat, U, prec)
+    F = lat.new_matrix_field(tdtype(prec))
+    qcd.qcd_gauge_force(lat, dU, F, beta)
+    assert rel(host(qcd, lat, F), Fr) < TOL[prec]
+    dP = dev(qcd, lat, P, prec)
+    qcd.qcd_force_mom_update(lat, dU, dP, beta, eps)
+    assert rel(host(qcd, lat, dP), P + eps * Fr) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 32)])
 def test_mom_update_and_fused_force_mom_update(qcd, orc_omp, prec, dims):
     lat = qcd.Lattice(dims)
