@@ -45,7 +45,7 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
 }
 
 // F_mu(x) for mu = 0..3 at the thread's site; FUSED: out = P, P += eps F; else out = F.
-template <typename T, bool FUSED, int PMODE>
+template <typename T, bool FUSED, bool EARLYP>
 __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out) {
@@ -60,19 +60,14 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         db[d] = dbwd(lat, st, d);
     }
 
-    if (FUSED && PMODE >= 2) {  // start pulling this thread's momenta towards the SM before the staple work
-#pragma unroll 4
-        for (int e = 0; e < 36; e++) {
-            if (PMODE == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(out + (size_t)e * V + cb));
-            else asm volatile("prefetch.global.L1 [%0];" ::"l"(out + (size_t)e * V + cb));
-        }
-    }
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
         const int dfm = mu == 0 ? df[0] : mu == 1 ? df[1] : mu == 2 ? df[2] : df[3];
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
         M3<T> A, Pm;
-        if (FUSED && PMODE == 1) load_link_rw(Pm, out, V, mu, cb);
+        // the momenta come straight from HBM (no reuse): issue their loads before the staple work so the
+        // DRAM latency is hidden behind it (measured: -9 % kernel time at 32^3x64 fp64)
+        if (FUSED && EARLYP) load_link_rw(Pm, out, V, mu, cb);
         zero(A);
 #pragma unroll
         for (int k = 1; k < 4; k++) {
@@ -103,7 +98,7 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         project_force(F, W, c);
         if (FUSED) {
             M3<T> P;
-            if (PMODE == 1) P = Pm;
+            if (EARLYP) P = Pm;
             else load_link_rw(P, out, V, mu, cb);
 #pragma unroll
             for (int e = 0; e < 9; e++) {
@@ -223,8 +218,9 @@ static TileP choose_tile(const LatP &lat, int subset, int target) {
                         const double vol = (double)t[0] * t[1] * t[2] * t[3];
                         double surf = 0;
                         for (int k = 0; k < 4; k++) surf += vol / t[k];
-                        // more threads first; then x extent up to 16 (128-byte rows in fp64); then compactness
-                        const double score = threads * 1e6 + (t[0] >= 16 ? 16 : t[0]) * 1e3 - surf / vol * 100.0;
+                        // more threads first; then x extent up to 32 (256-byte rows per parity in fp64; measured best on
+                        // B200, profiles/r01b_force_sweeps.md); then compactness
+                        const double score = threads * 1e6 + (t[0] >= 32 ? 32 : t[0]) * 1e3 - surf / vol * 100.0;
                         if (score > best_score) {
                             best_score = score;
                             memcpy(best, t, sizeof t);
@@ -250,12 +246,9 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
     if (site) {
         const TileP tp = choose_tile(lat->p, subset, 256);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
-        const char *pm = getenv("QCD_PMODE");
-        const int pmode = pm ? atoi(pm) : 0;
-        if (pmode == 1) force_kernel<T, FUSED, 1><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
-        else if (pmode == 2) force_kernel<T, FUSED, 2><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
-        else if (pmode == 3) force_kernel<T, FUSED, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
-        else force_kernel<T, FUSED, 0><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        const char *pm = getenv("QCD_EARLY_P");  // sweep knob; default on
+        if (!pm || atoi(pm)) force_kernel<T, FUSED, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        else force_kernel<T, FUSED, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
         return;
     }
     const char *t = getenv("QCD_FORCE_THREADS");
