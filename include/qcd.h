@@ -157,6 +157,20 @@ int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const v
 int qcd_md_step(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, void *U,
                 void *P, void *stream);
 
+/* The same MD step in ONE pass over the lattice (SURVEY.md 8(a) "single pass, ping-pong U"; loop fusion
+ * in the sense of PAPER.md:32): P <- P + eps_p*F(U_in); U_out <- reunit(exp(i eps_u P) U_in), one kernel.
+ * U_in is only read; U_out is a second gauge field of the same size that must not overlap U_in or P
+ * (QCD_EALIAS) because neighbouring sites still read the old links.  Results equal qcd_md_step's up to
+ * rounding order (same arithmetic per link). */
+int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
+                            const void *U_in, void *P, void *U_out, void *stream);
+
+/* Leapfrog trajectory [O11] built from single-pass steps: same result as qcd_leapfrog; U_work is a
+ * caller-owned scratch gauge field (qcd_field_bytes(lat, prec, 72) bytes) used as the ping-pong partner.
+ * The final links are always left in U (an odd nsteps starts with one two-kernel in-place step). */
+int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,
+                             void *P, void *U_work, void *stream);
+
 /* Leapfrog trajectory [O11]: P += (eps/2) F; n times { U <- reunit(exp(i eps P) U); P += eps F }
  * with eps/2 on the last. */
 int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,

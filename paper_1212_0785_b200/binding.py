@@ -40,6 +40,8 @@ SIGNATURES = {
     "qcd_sum_multi": (_i, [_vp, _i, _i, _i, _vp, _vp, _i, _vp, _vp, _vp]),
     "qcd_md_step": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp]),
     "qcd_leapfrog": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp]),
+    "qcd_md_step_single_pass": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp]),
+    "qcd_leapfrog_single_pass": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
     "qcd_pack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_unpack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_get_map": (_i, [_vp, _i, _vp, _vp]),
@@ -110,7 +112,7 @@ class Lattice:
 
     def __del__(self):
         h = getattr(self, "handle", None)
-        if h:
+        if h and lib is not None:  # `lib` is already None when the interpreter is shutting down
             lib.qcd_lattice_destroy(h)
             self.handle = None
 
@@ -182,6 +184,16 @@ def qcd_md_step(lat, U, P, beta, eps_p, eps_u, stream=None):
 
 def qcd_leapfrog(lat, U, P, beta, eps, nsteps, stream=None):
     _check(lib.qcd_leapfrog(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _stream(stream)))
+
+
+def qcd_md_step_single_pass(lat, U_in, P, U_out, beta, eps_p, eps_u, stream=None):
+    _check(lib.qcd_md_step_single_pass(lat.handle, _prec(U_in), beta, eps_p, eps_u, _ptr(U_in), _ptr(P), _ptr(U_out),
+                                       _stream(stream)))
+
+
+def qcd_leapfrog_single_pass(lat, U, P, U_work, beta, eps, nsteps, stream=None):
+    _check(lib.qcd_leapfrog_single_pass(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _ptr(U_work),
+                                        _stream(stream)))
 
 
 def qcd_pack(lat, ncomp, lex_aos, dev_soa, stream=None):

@@ -243,6 +243,50 @@ int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int 
     return QCD_OK;
 }
 
+int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
+                            const void *U_in, void *P, void *U_out, void *stream) {
+    const char *fn = "qcd_md_step_single_pass";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U_in, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U_out, fn));
+    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    QCD_TRY(check_alias(U_in, P, fb, fn));
+    QCD_TRY(check_alias(U_in, U_out, fb, fn));
+    QCD_TRY(check_alias(P, U_out, fb, fn));
+    return launch_md_single(lat, prec, beta, eps_p, eps_u, U_in, P, U_out, (cudaStream_t)stream);
+}
+
+int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,
+                             void *P, void *U_work, void *stream) {
+    const char *fn = "qcd_leapfrog_single_pass";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U_work, fn));
+    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    QCD_TRY(check_alias(U, P, fb, fn));
+    QCD_TRY(check_alias(U, U_work, fb, fn));
+    QCD_TRY(check_alias(P, U_work, fb, fn));
+    if (nsteps < 1) return bad(QCD_EINVAL, "%s: nsteps < 1", fn);
+    cudaStream_t st = (cudaStream_t)stream;
+    // O11 regrouped: n x { P += a_k F(U); U <- reunit(exp(i eps P) U) } with a_0 = eps/2, then P += (eps/2) F(U)
+    void *cur = U, *other = U_work;
+    int k = 0;
+    if (nsteps & 1) {  // keep the number of ping-pong steps even so the result lands in U
+        QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, U, P, true, st));
+        QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
+        k = 1;
+    }
+    for (; k < nsteps; k++) {
+        QCD_TRY(launch_md_single(lat, prec, beta, k == 0 ? 0.5 * eps : eps, eps, cur, P, other, st));
+        void *t = cur;
+        cur = other;
+        other = t;
+    }
+    return launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, cur, P, true, st);
+}
+
 int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream) {
     const char *fn = "qcd_pack";
     QCD_TRY(check_common(lat, prec, fn));

@@ -45,10 +45,14 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
 }
 
 // F_mu(x) for mu = 0..3 at the thread's site; FUSED: out = P, P += eps F; else out = F.
-template <typename T, bool FUSED, bool EARLYP>
-__global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
+// LINK (needs FUSED): the whole MD step in one pass over the lattice (SURVEY.md 8(a) "single pass, ping-pong U"):
+// with the updated momentum still in registers, Uout_mu(x) = reunit(exp(i eps_u P_mu(x)) U_mu(x)) is written
+// to a second gauge field (neighbouring threads still read the old U, so the update cannot be in place).
+template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1>
+__global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
-                                                    pair_t<T> *__restrict__ out) {
+                                                    pair_t<T> *__restrict__ out, const T eps_u,
+                                                    pair_t<T> *__restrict__ Uout) {
     const Site st = tile_site(lat, tile, threadIdx.x);
     const int V = lat.V;
     const int par = st.par;
@@ -67,7 +71,7 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         M3<T> A, Pm;
         // the momenta come straight from HBM (no reuse): issue their loads before the staple work so the
         // DRAM latency is hidden behind it (measured: -9 % kernel time at 32^3x64 fp64)
-        if (FUSED && EARLYP) load_link_rw(Pm, out, V, mu, cb);
+        if (FUSED && EARLYP) load_link_cs(Pm, out, V, mu, cb);
         zero(A);
 #pragma unroll
         for (int k = 1; k < 4; k++) {
@@ -99,7 +103,245 @@ __global__ void __launch_bounds__(256) force_kernel(const LatP lat, const TileP 
         if (FUSED) {
             M3<T> P;
             if (EARLYP) P = Pm;
-            else load_link_rw(P, out, V, mu, cb);
+            else load_link_cs(P, out, V, mu, cb);
+#pragma unroll
+            for (int e = 0; e < 9; e++) {
+                P.re[e] = fma_(eps, F.re[e], P.re[e]);
+                P.im[e] = fma_(eps, F.im[e], P.im[e]);
+            }
+            store_link_cs(P, out, V, mu, cb);
+            if (LINK) {
+#pragma unroll
+                for (int e = 0; e < 9; e++) {
+                    P.re[e] *= eps_u;
+                    P.im[e] *= eps_u;
+                }
+                M3<T> E, R;
+                expi_herm(E, P);
+                mul<false, false, false>(R, E, Um);
+                reunit(R);
+                store_link_cs(R, Uout, V, mu, cb);
+            }
+        } else {
+            store_link_cs(F, out, V, mu, cb);
+        }
+    }
+}
+
+// Variant "pipe": the same staple arithmetic as force_kernel, with the link loads software-pipelined by hand.
+// Each staple is Z = op(a) op(b); A += Z op(c).  With 254 registers only 8 warps are resident per SM, so a
+// wait on a group of loads is exposed; here the (a, b) links of the NEXT staple are requested before the
+// second product of the current one and c before its first product, so every load has one 3x3 product
+// (216 DFMA) of cover.  Live matrices at a product: A, Pm, Z, c and the two in flight = 216 registers (fp64).
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(256) force_pipe_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
+                                                         const T eps, const pair_t<T> *__restrict__ U,
+                                                         pair_t<T> *__restrict__ out) {
+    const Site st = tile_site(lat, tile, threadIdx.x);
+    const int V = lat.V;
+    const int par = st.par;
+    const int cb = cb_of(lat, st.s, par);
+    int df[4], db[4];
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+        df[d] = dfwd(lat, st, d);
+        db[d] = dbwd(lat, st, d);
+    }
+    auto fwd = [&](int d) { return d == 0 ? df[0] : d == 1 ? df[1] : d == 2 ? df[2] : df[3]; };
+    auto bwd = [&](int d) { return d == 0 ? db[0] : d == 1 ? db[1] : d == 2 ? db[2] : db[3]; };
+
+    M3<T> Xa, Xb;  // operands (a, b) of the next staple, in flight across loop iterations
+    load_link(Xa, U, V, 1, cb_of(lat, st.s + df[0], par ^ 1));  // mu = 0, nu = 1: U_nu(x+mu)
+    load_link(Xb, U, V, 0, cb_of(lat, st.s + df[1], par ^ 1));  //                 U_mu(x+nu)
+
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu++) {
+        const int dfm = fwd(mu);
+        const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
+        M3<T> A, Pm, Um, Z, C;
+        if (FUSED) load_link_rw(Pm, out, V, mu, cb);
+        zero(A);
+#pragma unroll
+        for (int k = 1; k < 4; k++) {
+            const int nu = (mu + k) & 3;
+            const int dbn = bwd(nu);
+            const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);  // x - nu
+            // up staple: U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+            load_link(C, U, V, nu, cb);
+            mul<false, true, false>(Z, Xa, Xb);
+            load_link(Xa, U, V, nu, cb_of(lat, st.s + dfm + dbn, par));  // U_nu(x+mu-nu)
+            load_link(Xb, U, V, mu, cb_mn);                              // U_mu(x-nu)
+            mul<false, true, true>(A, Z, C);
+            // down staple: U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu)
+            load_link(C, U, V, nu, cb_mn);
+            mul<true, true, false>(Z, Xa, Xb);
+            if (k < 3) {
+                const int nn = (mu + k + 1) & 3;
+                load_link(Xa, U, V, nn, cb_pm);                                   // U_nn(x+mu)
+                load_link(Xb, U, V, mu, cb_of(lat, st.s + fwd(nn), par ^ 1));     // U_mu(x+nn)
+            } else {
+                load_link(Um, U, V, mu, cb);
+            }
+            mul<false, false, true>(A, Z, C);
+        }
+        if (mu < 3) {  // first staple of the next direction: mu' = mu+1, nu' = mu+2
+            const int m1 = mu + 1, n1 = (mu + 2) & 3;
+            load_link(Xa, U, V, n1, cb_of(lat, st.s + fwd(m1), par ^ 1));
+            load_link(Xb, U, V, m1, cb_of(lat, st.s + fwd(n1), par ^ 1));
+        }
+        M3<T> W, F;
+        mul<false, false, false>(W, Um, A);
+        project_force(F, W, c);
+        if (FUSED) {
+#pragma unroll
+            for (int e = 0; e < 9; e++) {
+                Pm.re[e] = fma_(eps, F.re[e], Pm.re[e]);
+                Pm.im[e] = fma_(eps, F.im[e], Pm.im[e]);
+            }
+            store_link(Pm, out, V, mu, cb);
+        } else {
+            store_link(F, out, V, mu, cb);
+        }
+    }
+}
+
+// Variant "plane": the force assembled plane by plane from closed loops W = U_mu(x) * staple, so that the
+// (mu,nu) plaquette at x serves both F_mu(x) (+) and F_nu(x) (its dagger, -) and each own link starts two
+// chains: 10 link loads and 9 products per plane = 60 loads + 54 products per site instead of 80 + 52.
+// The kernel is bound by bytes through the L1 load path, so fewer loads is the lever.
+// Only the anti-Hermitian traceless part of each loop enters F (the projection is linear), so the four
+// accumulators are 9 reals each (3 diagonal imaginary parts, 3 complex off-diagonal differences).
+template <typename T>
+struct TAcc {
+    T d[3];   // sum Im W_ii
+    T xr[3];  // sum Re (W_ij - conj W_ji) for (ij) = (01), (02), (12)
+    T xi[3];  // sum Im (W_ij - conj W_ji)
+};
+
+template <typename T>
+__device__ __forceinline__ void tacc_zero(TAcc<T> &a) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) a.d[k] = a.xr[k] = a.xi[k] = T(0);
+}
+
+// a += sgn * antiHermitian part of W (sgn = -1 adds the part of W^dagger)
+template <int SGN, typename T>
+__device__ __forceinline__ void tacc_add(TAcc<T> &a, const M3<T> &W) {
+    const T s = T(SGN);
+#pragma unroll
+    for (int k = 0; k < 3; k++) a.d[k] += s * W.im[4 * k];
+    const int I[3] = {0, 0, 1}, J[3] = {1, 2, 2};
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        a.xr[k] += s * (W.re[3 * I[k] + J[k]] - W.re[3 * J[k] + I[k]]);
+        a.xi[k] += s * (W.im[3 * I[k] + J[k]] + W.im[3 * J[k] + I[k]]);
+    }
+}
+
+// F = (i c)[(W - W^dag) - tr/3] from the accumulated parts (same formulas as project_force)
+template <typename T>
+__device__ __forceinline__ void tacc_force(M3<T> &F, const TAcc<T> &a, T c) {
+    const T m = (a.d[0] + a.d[1] + a.d[2]) * T(1.0 / 3.0);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        F.re[4 * k] = T(-2) * c * (a.d[k] - m);
+        F.im[4 * k] = T(0);
+    }
+    const int I[3] = {0, 0, 1}, J[3] = {1, 2, 2};
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        F.re[3 * I[k] + J[k]] = -c * a.xi[k];
+        F.im[3 * I[k] + J[k]] = c * a.xr[k];
+        F.re[3 * J[k] + I[k]] = -c * a.xi[k];
+        F.im[3 * J[k] + I[k]] = -c * a.xr[k];
+    }
+}
+
+// all loops of the (mu,nu) plane through x that contain U_mu(x) or U_nu(x)
+template <typename T>
+__device__ __forceinline__ void plane_loops(TAcc<T> &am, TAcc<T> &an, const LatP &lat, const Site &st, int V,
+                                            const pair_t<T> *__restrict__ U, int mu, int nu, int dfm, int dbm,
+                                            int dfn, int dbn) {
+    const int par = st.par;
+    const int cb = cb_of(lat, st.s, par);
+    const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);  // x - nu
+    const int cb_mm = cb_of(lat, st.s + dbm, par ^ 1);  // x - mu
+    M3<T> Uo, B, M, N;
+    // lower loop of U_mu(x):  U_mu(x) U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu)
+    load_link(Uo, U, V, mu, cb);
+    load_link(B, U, V, nu, cb_of(lat, st.s + dfm + dbn, par));
+    mul<false, true, false>(M, Uo, B);
+    load_link(B, U, V, mu, cb_mn);
+    mul<false, true, false>(N, M, B);
+    load_link(B, U, V, nu, cb_mn);
+    mul<false, false, false>(M, N, B);
+    tacc_add<1>(am, M);
+    // plaquette:  U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag  -> +F_mu, its dagger -> F_nu
+    load_link(B, U, V, nu, cb_of(lat, st.s + dfm, par ^ 1));
+    mul<false, false, false>(M, Uo, B);
+    load_link(B, U, V, mu, cb_of(lat, st.s + dfn, par ^ 1));
+    mul<false, true, false>(N, M, B);
+    load_link(Uo, U, V, nu, cb);  // U_nu(x): closes the plaquette, then starts the lower loop of U_nu(x)
+    mul<false, true, false>(M, N, Uo);
+    tacc_add<1>(am, M);
+    tacc_add<-1>(an, M);
+    // lower loop of U_nu(x):  U_nu(x) U_mu(x+nu-mu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+    load_link(B, U, V, mu, cb_of(lat, st.s + dfn + dbm, par));
+    mul<false, true, false>(M, Uo, B);
+    load_link(B, U, V, nu, cb_mm);
+    mul<false, true, false>(N, M, B);
+    load_link(B, U, V, mu, cb_mm);
+    mul<false, false, false>(M, N, B);
+    tacc_add<1>(an, M);
+}
+
+template <typename T, bool FUSED>
+__global__ void __launch_bounds__(256) force_plane_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
+                                                          const T eps, const pair_t<T> *__restrict__ U,
+                                                          pair_t<T> *__restrict__ out) {
+    const Site st = tile_site(lat, tile, threadIdx.x);
+    const int V = lat.V;
+    const int cb = cb_of(lat, st.s, st.par);
+    int df[4], db[4];
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+        df[d] = dfwd(lat, st, d);
+        db[d] = dbwd(lat, st, d);
+    }
+    // a0..a3 belong to directions mu, mu+1, mu+2, mu+3 (mod 4) of the current iteration: the accumulators
+    // rotate by register moves so that the loop body is compiled once
+    TAcc<T> a0, a1, a2, a3;
+    tacc_zero(a0);
+    tacc_zero(a1);
+    tacc_zero(a2);
+    tacc_zero(a3);
+#pragma unroll 1
+    for (int mu = 0; mu < 4; mu++) {
+        const int n1 = (mu + 1) & 3, n2 = (mu + 2) & 3;
+        const int dfm = mu == 0 ? df[0] : mu == 1 ? df[1] : mu == 2 ? df[2] : df[3];
+        const int dbm = mu == 0 ? db[0] : mu == 1 ? db[1] : mu == 2 ? db[2] : db[3];
+        const int df1 = n1 == 0 ? df[0] : n1 == 1 ? df[1] : n1 == 2 ? df[2] : df[3];
+        const int db1 = n1 == 0 ? db[0] : n1 == 1 ? db[1] : n1 == 2 ? db[2] : db[3];
+        plane_loops(a0, a1, lat, st, V, U, mu, n1, dfm, dbm, df1, db1);  // planes (0,1) (1,2) (2,3) (3,0)
+        if (mu < 2) {                                                      // planes (0,2) (1,3)
+            const int df2 = n2 == 0 ? df[0] : n2 == 1 ? df[1] : n2 == 2 ? df[2] : df[3];
+            const int db2 = n2 == 0 ? db[0] : n2 == 1 ? db[1] : n2 == 2 ? db[2] : db[3];
+            plane_loops(a0, a2, lat, st, V, U, mu, n2, dfm, dbm, df2, db2);
+        }
+        const TAcc<T> t = a0;
+        a0 = a1;
+        a1 = a2;
+        a2 = a3;
+        a3 = t;
+    }
+    // after four rotations a_k is direction k again
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        M3<T> F;
+        tacc_force(F, mu == 0 ? a0 : mu == 1 ? a1 : mu == 2 ? a2 : a3, c);
+        if (FUSED) {
+            M3<T> P;
+            load_link_rw(P, out, V, mu, cb);
 #pragma unroll
             for (int e = 0; e < 9; e++) {
                 P.re[e] = fma_(eps, F.re[e], P.re[e]);
@@ -236,19 +478,41 @@ static TileP choose_tile(const LatP &lat, int subset, int target) {
 }
 
 // QCD_FORCE_VARIANT selects the kernel for block-shape / mapping sweeps (the paper's N_t tuning,
-// PAPER.md:57): "site" = one thread per site (256 threads), "link" = one thread per (site, mu) with
-// QCD_FORCE_THREADS in {256, 512} threads per block.
+// PAPER.md:57): "site" (default) = one thread per site, 128-thread blocks; "site256" = the same kernel in
+// 256-thread blocks with the momenta loaded early; "pipe" / "plane" = the hand-pipelined and the plane-wise
+// kernels above; "link" = one thread per (site, mu) with QCD_FORCE_THREADS in {256, 512} threads per block.
 template <typename T, bool FUSED>
 static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const pair_t<T> *U, pair_t<T> *out,
                            cudaStream_t st) {
     const char *v = getenv("QCD_FORCE_VARIANT");
-    const bool site = !v || strcmp(v, "link");
-    if (site) {
+    if (!v || strcmp(v, "site256") && strcmp(v, "plane") && strcmp(v, "pipe") && strcmp(v, "link")) {
+        // default: 128-thread blocks, three per SM (168 registers in fp64, 12 warps/SM); measured best at
+        // 32^3x64 in both precisions (profiles/r01c_force_sweeps.md)
+        const TileP tp = choose_tile(lat->p, subset, 128);
+        const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+        force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+        return;
+    }
+    if (!strcmp(v, "site256")) {  // 256-thread blocks, one per SM in fp64 (254 registers), momenta loaded early
         const TileP tp = choose_tile(lat->p, subset, 256);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         const char *pm = getenv("QCD_EARLY_P");  // sweep knob; default on
-        if (!pm || atoi(pm)) force_kernel<T, FUSED, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
-        else force_kernel<T, FUSED, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        if (!pm || atoi(pm))
+            force_kernel<T, FUSED, true, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+        else
+            force_kernel<T, FUSED, false, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+        return;
+    }
+    if (!strcmp(v, "plane")) {
+        const TileP tp = choose_tile(lat->p, subset, 256);
+        const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+        force_plane_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
+        return;
+    }
+    if (!strcmp(v, "pipe")) {
+        const TileP tp = choose_tile(lat->p, subset, 256);
+        const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+        force_pipe_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
         return;
     }
     const char *t = getenv("QCD_FORCE_THREADS");
@@ -269,8 +533,25 @@ static int launch_force_t(const qcd_lattice *lat, int subset, double beta, doubl
     return check_launch(fused ? "force_mom_update" : "gauge_force");
 }
 
+// Single-pass MD step: P += eps_p F(U); Uout = reunit(exp(i eps_u P) U).  Subset ALL only (every link moves).
+template <typename T>
+static int launch_md_single_t(const qcd_lattice *lat, double beta, double eps_p, double eps_u, const void *U, void *P,
+                              void *Uout, cudaStream_t st) {
+    const TileP tp = choose_tile(lat->p, QCD_ALL, 128);
+    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+    force_kernel<T, true, false, true, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(
+        lat->p, tp, (T)(beta / 12.0), (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u, (pair_t<T> *)Uout);
+    return check_launch("md_step_single_pass");
+}
+
+int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
+                     void *Uout, cudaStream_t st) {
+    return prec == QCD_F64 ? launch_md_single_t<double>(lat, beta, eps_p, eps_u, U, P, Uout, st)
+                           : launch_md_single_t<float>(lat, beta, eps_p, eps_u, U, P, Uout, st);
+}
+
 // Kernel choice.  Default: the plain staple kernels of this file (the definition, valid for arbitrary 3x3
-// matrices and for subsets).  QCD_FORCE_VARIANT = site | link | tile | plaq selects a variant for the
+// matrices and for subsets).  QCD_FORCE_VARIANT = site | site256 | pipe | plane | link | tile | plaq selects a variant for the
 // block-shape / mapping sweeps (the paper's N_t auto-tuning); tile (force_tile.cu) and plaq
 // (force_plaq.cu, needs unitary links) exist for subset ALL only.  DESIGN.md section 6 has the measurements.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,

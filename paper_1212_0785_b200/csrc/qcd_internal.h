@@ -53,6 +53,9 @@ int check_launch(const char *what);
 // kernel launchers, one per translation unit; prec already validated. All return QCD_OK/QCD_ECUDA.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
                        void *out, bool fused_mom, cudaStream_t st);
+// single-pass MD step (force.cu): P += eps_p F(U); Uout = reunit(exp(i eps_u P) U); U and Uout distinct
+int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
+                     void *Uout, cudaStream_t st);
 // plaquette-sharing force kernel (force_plaq.cu): subset ALL, unitary links
 int launch_gauge_force_plaq(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *out,
                             bool fused_mom, cudaStream_t st);

@@ -38,6 +38,31 @@ __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict_
     }
 }
 
+// streaming variants (ld.global.cs / st.global.cs): for data touched once per kernel (the momenta in the
+// force kernel), so that it does not displace the neighbour links other threads of the block reuse from L1
+template <typename T>
+__device__ __forceinline__ void load_link_cs(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {
+    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        pair_t<T> v = __ldcs(p + (size_t)e * V);
+        m.re[e] = v.x;
+        m.im[e] = v.y;
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ void store_link_cs(const M3<T> &m, pair_t<T> *f, int V, int mu, int cb) {
+    pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        pair_t<T> v;
+        v.x = m.re[e];
+        v.y = m.im[e];
+        __stcs(p + (size_t)e * V, v);
+    }
+}
+
 // same, through the normal (coherent) path: for fields the kernel also writes
 template <typename T>
 __device__ __forceinline__ void load_link_rw(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {

@@ -266,7 +266,8 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("link", None), ("tile", None),
+@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("site256", None), ("site256", "4,2,2,2"), ("pipe", None), ("pipe", "4,2,2,2"),
+                                          ("plane", None), ("plane", "4,2,2,2"), ("link", None), ("tile", None),
                                           ("tile", "8,2,2,4"), ("tile", "4,4,4,4"), ("plaq", None),
                                           ("plaq", "8,4,2,2"), ("plaq", "4,2,4,2")])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 4), (16, 8, 8, 16)])
@@ -461,6 +462,51 @@ def test_config2_trajectory_parity_each_step_and_reversibility(qcd, orc_omp):
     assert rel(host(qcd, lat, dP), P0) < 1e-12
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 4, 4, 4), (6, 4, 2, 8), (12, 6, 10, 4), (16, 16, 16, 32)])
+def test_md_step_single_pass(qcd, orc_omp, prec, dims):
+    """the one-kernel MD step (force + momentum + exp + reunit, ping-pong U) against the oracle's three steps"""
+    beta, eps_p, eps_u = 5.7, 0.03, 0.07
+    lat = qcd.Lattice(dims)
+    U = round_to(prec, orc_omp.hot_start(dims, 41, 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, 42))
+    dU, dP = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec)
+    dV = lat.new_matrix_field(tdtype(prec))
+    dV.fill_(float("nan"))
+    keep = dU.clone()
+    qcd.qcd_md_step_single_pass(lat, dU, dP, dV, beta, eps_p, eps_u)
+    P1 = orc_omp.mom_update(dims, eps_p, orc_omp.gauge_force(dims, beta, U), P)
+    U1 = orc_omp.link_update(dims, eps_u, P1, U, reunit=True)
+    assert rel(host(qcd, lat, dP), P1) < TOL[prec]
+    assert rel(host(qcd, lat, dV), U1) < TOL[prec]
+    import torch
+    assert torch.equal(dU, keep)  # the input links are only read
+    # aliasing is refused
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.qcd_md_step_single_pass(lat, dU, dP, dU, beta, eps_p, eps_u)
+    assert e.value.code == qcd.EALIAS
+
+
+@pytest.mark.parametrize("prec,nsteps", [("f64", 1), ("f64", 4), ("f64", 5), ("f32", 3)])
+def test_leapfrog_single_pass_matches_oracle_trajectory(qcd, orc_omp, prec, nsteps):
+    c = inputs.CONFIGS[2]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    seed = inputs.config_seed(2)
+    lat = qcd.Lattice(dims)
+    U = round_to(prec, orc_omp.hot_start(dims, seed, c["sigma"]))
+    P = round_to(prec, orc_omp.mom_refresh(dims, seed))
+    dU, dP = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec)
+    dW = lat.new_matrix_field(tdtype(prec))
+    qcd.qcd_leapfrog_single_pass(lat, dU, dP, dW, beta, eps, nsteps)
+    U1, P1 = orc_omp.leapfrog(dims, beta, eps, nsteps, U, P)
+    assert rel(host(qcd, lat, dU), U1) < TOL[prec] and rel(host(qcd, lat, dP), P1) < TOL[prec]
+    if prec == "f64":  # reversibility through the same driver
+        dP.mul_(-1.0)
+        qcd.qcd_leapfrog_single_pass(lat, dU, dP, dW, beta, eps, nsteps)
+        dP.mul_(-1.0)
+        assert rel(host(qcd, lat, dU), U) < 1e-12 and rel(host(qcd, lat, dP), P) < 1e-12
+
+
 def test_fp32_trajectory_tracks_fp64_oracle(qcd, orc_omp):
     c = inputs.CONFIGS[2]
     dims, beta, eps = c["dims"], c["beta"], c["eps"]
@@ -490,8 +536,8 @@ def sample_sites(dims, n, seed):
     return np.unique(np.array(pts, dtype=np.int32))
 
 
-@pytest.mark.parametrize("cfg,prec", [(4, "f64"), (5, "f32")])
-def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec):
+@pytest.mark.parametrize("cfg,prec,single", [(4, "f64", False), (4, "f64", True), (5, "f32", False)])
+def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
     """BASELINE configs 4 (32^3x64 fp64, the headline) and 5 (48^3x96): the fused MD step exactly as
     bench.py launches it (qcd_md_step, subset ALL), checked at sampled sites the oracle computes one
     by one, plus properties that hold at any size."""
@@ -535,8 +581,13 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec):
     rplaq, rper_t = orc_omp.plaquette(dims, U0)
     assert abs(plaq.item() - rplaq) / rplaq < TOL[prec]
     assert rel(per_t.cpu().numpy(), rper_t) < TOL[prec]
-    # one fused MD step
-    qcd.qcd_md_step(lat, dU, dP, beta, eps, eps)
+    # one fused MD step (two kernels in place, or the single-pass kernel writing a second gauge field)
+    if single:
+        dV = lat.new_matrix_field(dt)
+        qcd.qcd_md_step_single_pass(lat, dU, dP, dV, beta, eps, eps)
+        dU = dV
+    else:
+        qcd.qcd_md_step(lat, dU, dP, beta, eps, eps)
     Fs = orc_omp.gauge_force_sites(dims, beta, U0, sites)
     P1 = Psites + eps * Fs
     assert rel(gather(dP), P1) < TOL[prec]
