@@ -31,7 +31,9 @@ CONFIGS = {  # BASELINE.json configs: dims, hot-start sigma, beta, eps
     4: dict(dims=(32, 32, 32, 64), sigma=0.2, beta=6.0, eps=0.02, name="32^3x64"),
     5: dict(dims=(48, 48, 48, 96), sigma=0.3, beta=6.2, eps=0.01, name="48^3x96"),
 }
-BYTES_PER_SITE = {"force_mom_update": 216, "link_update_reunit": 216}  # reals/site R+W
+# reals/site R+W: force+mom reads U,P writes P; exp+reunit reads P,U writes U; the single-pass
+# kernel reads U,P and writes P,U
+BYTES_PER_SITE = {"force_mom_update": 216, "link_update_reunit": 216, "md_step_single_pass": 288}
 METRIC = "md_step_site_updates_per_s"
 UNIT = "site-updates/s"
 
@@ -161,8 +163,31 @@ def run_ours(args, cfg):
     qcd.qcd_mom_refresh(lat, P, SEED_BASE + 4 + 1000 * rank)
     stream = torch.cuda.current_stream()
 
-    for _ in range(args.warmup):
-        qcd.qcd_md_step(lat, U, P, beta, eps, eps)
+    single = args.path == "single_pass"
+    bufs = [U, lat.new_matrix_field(dtype)] if single else [U]
+
+    def step(k, ev=None):
+        """one MD step; k counts steps (the single-pass kernel ping-pongs between two gauge fields)"""
+        if single:
+            if ev:
+                ev[0].record(stream)
+            qcd.qcd_md_step_single_pass(lat, bufs[k & 1], P, bufs[(k + 1) & 1], beta, eps, eps)
+            if ev:
+                ev[1].record(stream)
+                ev[2].record(stream)
+        else:
+            if ev:
+                ev[0].record(stream)
+            qcd.qcd_force_mom_update(lat, U, P, beta, eps)
+            if ev:
+                ev[1].record(stream)
+            qcd.qcd_link_update(lat, P, U, eps, reunit=True)
+            if ev:
+                ev[2].record(stream)
+
+    nwarm = args.warmup + (args.warmup & 1 if single else 0)  # even, so the timed steps start from bufs[0]
+    for k in range(nwarm):
+        step(k)
     try:  # NVML index of this CUDA device (differs from `local` under CUDA_VISIBLE_DEVICES)
         nvml_index = torch.cuda._get_nvml_device_index(local)
     except Exception:  # noqa: BLE001
@@ -176,11 +201,7 @@ def run_ours(args, cfg):
     barrier()
     sampler.active = True
     for k in range(K):
-        ev[k][0].record(stream)
-        qcd.qcd_force_mom_update(lat, U, P, beta, eps)
-        ev[k][1].record(stream)
-        qcd.qcd_link_update(lat, P, U, eps, reunit=True)
-        ev[k][2].record(stream)
+        step(k, ev[k])
     barrier()
     sampler.active = False
     elapsed_ms = ev[0][0].elapsed_time(ev[K - 1][2])
@@ -225,30 +246,34 @@ def run_ours(args, cfg):
         return
 
     peak, peak_src = peaks()
-    force_bytes = BYTES_PER_SITE["force_mom_update"] * rbytes * V
+    top = "md_step_single_pass" if single else "force_mom_update"
+    force_bytes = BYTES_PER_SITE[top] * rbytes * V
+    step_bytes = force_bytes if single else 2 * force_bytes
     achieved = force_bytes / (force_ms * 1e-3) / 1e9
     traffic = None
     tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"force_mom_update_{args.dtype}_{cfg['name']}")
+        traffic = json.load(open(tp)).get(f"{top}_{args.dtype}_{cfg['name']}")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
         "ms_per_step": elapsed_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": f"{cfg['name']} {'fp64' if args.dtype == 'f64' else 'fp32'} fused MD step "
-                               f"(force+momentum, exp+reunit), sigma={cfg['sigma']} beta={beta} eps={eps}",
+                               f"({'one single-pass kernel' if single else 'force+momentum, exp+reunit'}), sigma={cfg['sigma']} beta={beta} eps={eps}",
                    "sites_per_gpu": V, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                    "l2": f"inputs U+P = {2 * fb / 1e6:.0f} MB per GPU, larger than the 126 MB L2: no flush needed"
                          if 2 * fb > 2 * 126e6 else "inputs fit L2: numbers are L2-resident, not HBM",
-                   "step_hbm_gbs": 2 * force_bytes / (elapsed_ms / K * 1e-3) / 1e9,
-                   "step_frac_of_hbm_peak": 2 * force_bytes / (elapsed_ms / K * 1e-3) / 1e9 / peak,
-                   "kernel_ms": {"force_mom_update": force_ms, "link_update_reunit": link_ms}},
-        "roofline": {"bound": "hbm", "kernel": "force_mom_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                   "path": args.path,
+                   "step_hbm_gbs": step_bytes / (elapsed_ms / K * 1e-3) / 1e9,
+                   "step_frac_of_hbm_peak": step_bytes / (elapsed_ms / K * 1e-3) / 1e9 / peak,
+                   "kernel_ms": {top: force_ms} if single else
+                                {"force_mom_update": force_ms, "link_update_reunit": link_ms}},
+        "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": force_bytes},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * fb, "d2h_bytes_per_step": 2 * fb,
                 "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout)"},
-        "gpu_launches": 2 * K,
+        "gpu_launches": K if single else 2 * K,
         "clocks": sampler.summary(),
     }
     if world == 1 and not args.no_cpu_baseline:
@@ -272,6 +297,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--path", default="two_kernel", choices=["two_kernel", "single_pass"],
+                    help="two_kernel: qcd_force_mom_update + qcd_link_update(reunit) in place (default, the faster "
+                         "one as measured); single_pass: qcd_md_step_single_pass ping-ponging two gauge fields")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -48,7 +48,13 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
 // LINK (needs FUSED): the whole MD step in one pass over the lattice (SURVEY.md 8(a) "single pass, ping-pong U"):
 // with the updated momentum still in registers, Uout_mu(x) = reunit(exp(i eps_u P_mu(x)) U_mu(x)) is written
 // to a second gauge field (neighbouring threads still read the old U, so the update cannot be in place).
-template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1>
+template <bool REC, typename T>
+__device__ __forceinline__ void ldU(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
+    if (REC) load_link_su3(m, f, V, mu, cb);
+    else load_link(m, f, V, mu, cb);
+}
+
+template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1, bool REC = false>
 __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out, const T eps_u,
@@ -83,20 +89,20 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
             const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
             M3<T> X, Y, Z;
             // up staple: U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
-            load_link(X, U, V, nu, cb_pm);
-            load_link(Y, U, V, mu, cb_pn);
+            ldU<REC>(X, U, V, nu, cb_pm);
+            ldU<REC>(Y, U, V, mu, cb_pn);
             mul<false, true, false>(Z, X, Y);
-            load_link(X, U, V, nu, cb);
+            ldU<REC>(X, U, V, nu, cb);
             mul<false, true, true>(A, Z, X);
             // down staple: U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu)
-            load_link(X, U, V, nu, cb_pmmn);
-            load_link(Y, U, V, mu, cb_mn);
+            ldU<REC>(X, U, V, nu, cb_pmmn);
+            ldU<REC>(Y, U, V, mu, cb_mn);
             mul<true, true, false>(Z, X, Y);
-            load_link(X, U, V, nu, cb_mn);
+            ldU<REC>(X, U, V, nu, cb_mn);
             mul<false, false, true>(A, Z, X);
         }
         M3<T> Um, W;
-        load_link(Um, U, V, mu, cb);
+        ldU<REC>(Um, U, V, mu, cb);
         mul<false, false, false>(W, Um, A);
         M3<T> F;
         project_force(F, W, c);
@@ -490,7 +496,10 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
         // 32^3x64 in both precisions (profiles/r01c_force_sweeps.md)
         const TileP tp = choose_tile(lat->p, subset, 128);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
-        force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+        if (getenv("QCD_SU3_REC"))  // sweep knob: SU(3) links only (two-row loads); measured no gain, off by default
+            force_kernel<T, FUSED, false, false, 128, 3, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+        else
+            force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
         return;
     }
     if (!strcmp(v, "site256")) {  // 256-thread blocks, one per SM in fp64 (254 registers), momenta loaded early

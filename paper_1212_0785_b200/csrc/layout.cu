@@ -20,6 +20,69 @@ __global__ void __launch_bounds__(256) pack_kernel(const LatP lat, const int nco
     }
 }
 
+// Same maps through a shared-memory transpose, so that both sides are coalesced: a block takes PK_SITES
+// consecutive lexicographic sites (one contiguous chunk of the canonical array, both parities) and the
+// matching PK_SITES/2 consecutive checkerboard indices of each parity (pair h = s>>1 holds one even and one
+// odd site because Lx is even).  Site stride in shared memory is ncomp+2 reals (bank spread).
+constexpr int PK_SITES = 64;
+
+template <typename T, bool UNPACK>
+__global__ void __launch_bounds__(256) pack_tr_kernel(const LatP lat, const int ncomp, const bool matrix,
+                                                      const T *__restrict__ src, T *__restrict__ dst) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sm = reinterpret_cast<T *>(smem_raw);
+    const int ss = ncomp + 2;
+    const int s0 = blockIdx.x * PK_SITES;
+    const int ns = min(PK_SITES, lat.V - s0);  // V is even and s0 is even: ns is even
+    const int nh = ns >> 1;
+    const int h0 = s0 >> 1;
+    const int nel = ns * ncomp;
+    const T *aos_in = UNPACK ? nullptr : src + (size_t)s0 * ncomp;
+    T *aos_out = UNPACK ? dst + (size_t)s0 * ncomp : nullptr;
+    if (!UNPACK)
+        for (int i = threadIdx.x; i < nel; i += blockDim.x) sm[(i / ncomp) * ss + i % ncomp] = aos_in[i];
+    else {
+        // checkerboard side -> shared
+        for (int i = threadIdx.x; i < nel; i += blockDim.x) {
+            // i = ((c2 * 2 + par) * nh + hl) * w + ri, w = 2 reals (matrix) or 1
+            const int w = matrix ? 2 : 1;
+            const int ri = i % w;
+            int r = i / w;
+            const int hl = r % nh;
+            r /= nh;
+            const int par = r & 1;
+            const int c = (r >> 1) * w + ri;
+            const int h = h0 + hl;
+            const int row = (2 * h) / lat.L[0];
+            const int y = row % lat.L[1], zt = row / lat.L[1];
+            const int odd = (y + zt % lat.L[2] + zt / lat.L[2] + par) & 1;
+            const int cb = par * lat.Vh + h;
+            const size_t soa = matrix ? 2 * ((size_t)(c >> 1) * lat.V + cb) + (c & 1) : (size_t)c * lat.V + cb;
+            sm[(2 * hl + odd) * ss + c] = src[soa];
+        }
+    }
+    __syncthreads();
+    if (UNPACK)
+        for (int i = threadIdx.x; i < nel; i += blockDim.x) aos_out[i] = sm[(i / ncomp) * ss + i % ncomp];
+    else
+        for (int i = threadIdx.x; i < nel; i += blockDim.x) {
+            const int w = matrix ? 2 : 1;
+            const int ri = i % w;
+            int r = i / w;
+            const int hl = r % nh;
+            r /= nh;
+            const int par = r & 1;
+            const int c = (r >> 1) * w + ri;
+            const int h = h0 + hl;
+            const int row = (2 * h) / lat.L[0];
+            const int y = row % lat.L[1], zt = row / lat.L[1];
+            const int odd = (y + zt % lat.L[2] + zt / lat.L[2] + par) & 1;
+            const int cb = par * lat.Vh + h;
+            const size_t soa = matrix ? 2 * ((size_t)(c >> 1) * lat.V + cb) + (c & 1) : (size_t)c * lat.V + cb;
+            dst[soa] = sm[(2 * hl + odd) * ss + c];
+        }
+}
+
 __global__ void map_kernel(const LatP lat, const int which, int32_t *__restrict__ out) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= lat.V) return;
@@ -36,6 +99,19 @@ __global__ void map_kernel(const LatP lat, const int which, int32_t *__restrict_
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *src, void *dst, bool unpack,
                 cudaStream_t st) {
     const bool matrix = ncomp % 18 == 0;
+    const size_t rb = prec == QCD_F64 ? 8 : 4;
+    const size_t shm = (size_t)PK_SITES * (ncomp + 2) * rb;
+    if (shm <= 48 * 1024) {  // transpose through shared memory; larger ncomp falls back to the direct kernel
+        const int blocks = (lat->p.V + PK_SITES - 1) / PK_SITES;
+        if (prec == QCD_F64) {
+            if (unpack) pack_tr_kernel<double, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);
+            else pack_tr_kernel<double, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);
+        } else {
+            if (unpack) pack_tr_kernel<float, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst);
+            else pack_tr_kernel<float, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst);
+        }
+        return check_launch(unpack ? "unpack" : "pack");
+    }
     const dim3 grid((lat->p.V + 255) / 256, ncomp < 72 ? ncomp : 72);
     if (prec == QCD_F64) {
         if (unpack) pack_kernel<double, true><<<grid, 256, 0, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);

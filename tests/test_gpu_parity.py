@@ -97,9 +97,10 @@ def test_rng_words_and_uniforms_bit_exact(qcd, orc):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_pack_unpack_layout(qcd, orc, prec):
+@pytest.mark.parametrize("dims", [(4, 6, 2, 4), (2, 2, 2, 2), (4, 10, 6, 2), (16, 8, 8, 6)])
+def test_pack_unpack_layout(qcd, orc, prec, dims):
+    """bit-exact; V = 192, 16, 480, 6144: whole 64-site chunks of the transposing kernel and ragged tails"""
     import torch
-    dims = (4, 6, 2, 4)
     lat = qcd.Lattice(dims)
     V = lat.V
     A = round_to(prec, inputs.random_matrix_field(3, V))
@@ -120,6 +121,18 @@ def test_pack_unpack_layout(qcd, orc, prec):
     qcd.qcd_pack(lat, 3, src, dst)
     got = dst.cpu().numpy().astype(np.float64)
     assert np.array_equal(got[:, cb], R.T)
+    back = torch.empty_like(src)
+    qcd.qcd_unpack(lat, 3, dst, back)
+    assert torch.equal(back, src)
+    # many components per site: the direct (non-transposing) kernel
+    R = round_to(prec, inputs.random_real_field(5, V, 100))
+    src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
+    dst = lat.new_real_field(100, tdtype(prec))
+    qcd.qcd_pack(lat, 100, src, dst)
+    assert np.array_equal(dst.cpu().numpy().astype(np.float64)[:, cb], R.T)
+    back = torch.empty_like(src)
+    qcd.qcd_unpack(lat, 100, dst, back)
+    assert torch.equal(back, src)
 
 
 # ------------------------------------------------------------------ generators
@@ -266,7 +279,8 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("site256", None), ("site256", "4,2,2,2"), ("pipe", None), ("pipe", "4,2,2,2"),
+@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("site+rec", None), ("site256", None),
+                                          ("site256", "4,2,2,2"), ("pipe", None), ("pipe", "4,2,2,2"),
                                           ("plane", None), ("plane", "4,2,2,2"), ("link", None), ("tile", None),
                                           ("tile", "8,2,2,4"), ("tile", "4,4,4,4"), ("plaq", None),
                                           ("plaq", "8,4,2,2"), ("plaq", "4,2,4,2")])
@@ -275,6 +289,9 @@ def test_force_kernel_variants(qcd, orc_omp, monkeypatch, prec, variant, tile, d
     """every selectable force kernel (QCD_FORCE_VARIANT, QCD_TILE: the block-shape sweep knobs) against the
     oracle, fused and unfused, on SU(3) links (the plaq variant needs unitary links), over several tiles
     and with tiles that span a whole extent (periodic wrap inside the tile)"""
+    if variant.endswith("+rec"):  # two-row loads of SU(3) links (third row rebuilt in registers)
+        variant = variant[:-4]
+        monkeypatch.setenv("QCD_SU3_REC", "1")
     monkeypatch.setenv("QCD_FORCE_VARIANT", variant)
     if tile:
         if any(d % t for d, t in zip(dims, map(int, tile.split(",")))):
