@@ -133,6 +133,22 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def replica_seed(rank):
+    """each replica (rank) runs its own lattice: distinct hot-start / momentum seeds"""
+    return SEED_BASE + 4 + 1000 * rank
+
+
+def aggregate(elapsed_ms, sites_per_rank, steps, world, device):
+    """whole-job throughput from per-rank device times: MAX elapsed over ranks (one all-reduce, outside the
+    timed region), value = world x sites x steps / that time.  Returns (value, max_elapsed_ms)."""
+    import torch
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return world * sites_per_rank * steps / (t.item() * 1e-3), t.item()
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -159,8 +175,8 @@ def run_ours(args, cfg):
     lat = qcd.Lattice(dims)
     V = lat.V
     U, P = lat.new_matrix_field(dtype), lat.new_matrix_field(dtype)
-    qcd.qcd_hot_start(lat, U, SEED_BASE + 4 + 1000 * rank, cfg["sigma"])
-    qcd.qcd_mom_refresh(lat, P, SEED_BASE + 4 + 1000 * rank)
+    qcd.qcd_hot_start(lat, U, replica_seed(rank), cfg["sigma"])
+    qcd.qcd_mom_refresh(lat, P, replica_seed(rank))
     stream = torch.cuda.current_stream()
 
     single = args.path == "single_pass"
@@ -207,11 +223,7 @@ def run_ours(args, cfg):
     elapsed_ms = ev[0][0].elapsed_time(ev[K - 1][2])
     force_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / K
     link_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / K
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    elapsed_ms = t.item()
-    value = world * V * K / (elapsed_ms * 1e-3)
+    value, elapsed_ms = aggregate(elapsed_ms, V, K, world, "cuda")
 
     # ---- e2e: the C-ABI call on HOST buffers (pinned), H2D + pack + step + unpack + D2H every step
     Ke = max(1, min(K, args.e2e_steps))
@@ -234,10 +246,7 @@ def run_ours(args, cfg):
         stream.synchronize()  # the caller reads the step's result on the host
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * V * Ke / (t.item() * 1e-3)
+    e2e_value, _ = aggregate(e0.elapsed_time(e1), V, Ke, world, "cuda")
     sampler.stop_flag = True
 
     if rank != 0:
