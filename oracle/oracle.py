@@ -58,6 +58,10 @@ class Oracle:
         L.orc_hamiltonian.argtypes = [_c_int4, C.c_double, _dp, _dp, _dp, _dp]
         L.orc_leapfrog.argtypes = [_c_int4, C.c_double, C.c_double, C.c_int, _dp, _dp]
         L.orc_md_step.argtypes = [_c_int4, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_plaquette_st.argtypes = [_c_int4, _dp, _dp, _dp]
+        L.orc_action_aniso.argtypes = [_c_int4, C.c_double, C.c_double, _dp, _dp]
+        L.orc_gauge_force_aniso.argtypes = [_c_int4, C.c_int, C.c_double, C.c_double, _dp, _dp]
+        L.orc_nested_leapfrog.argtypes = [_c_int4, _dp, _dp, C.c_double, C.c_int, C.c_int, _dp, _dp]
         L.orc_map.argtypes = [_c_int4, C.c_int, C.POINTER(C.c_int32)]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
         L.orc_philox4x32_10.restype = None
@@ -234,6 +238,35 @@ class Oracle:
         out = np.empty((nsub, ncomp) if kind == SUM_SCALAR else (nsub,))
         self._ok(self.lib.orc_sum_multi(_c_int4(*dims), kind, ncomp, _ptr(f), idp, nsub, _ptr(out)), "sum_multi")
         return out
+
+    # ---- O13 anisotropic Wilson action, O14 two-level leapfrog
+    def plaquette_st(self, dims, U):
+        """(avg[2], per_t[Lt,2]): space-space and space-time plaquette averages"""
+        avg, per_t = np.empty(2), np.empty((dims[3], 2))
+        self._ok(self.lib.orc_plaquette_st(_c_int4(*dims), _mat(U, self.volume(dims)), _ptr(avg), _ptr(per_t)), "plaq_st")
+        return avg, per_t
+
+    def action_aniso(self, dims, beta_s, beta_t, U):
+        S = np.empty(1)
+        self._ok(self.lib.orc_action_aniso(_c_int4(*dims), beta_s, beta_t, _mat(U, self.volume(dims)), _ptr(S)),
+                 "action_aniso")
+        return float(S[0])
+
+    def gauge_force_aniso(self, dims, beta_s, beta_t, U, subset=ALL, out=None):
+        V = self.volume(dims)
+        F = np.zeros_like(U) if out is None else out
+        self._ok(self.lib.orc_gauge_force_aniso(_c_int4(*dims), subset, beta_s, beta_t, _mat(U, V), _mat(F, V)),
+                 "gauge_force_aniso")
+        return F
+
+    def nested_leapfrog(self, dims, bs, bt, tau, n_outer, n_inner, U, P):
+        """bs, bt: (level 0 = inner, level 1 = outer) coefficients"""
+        V = self.volume(dims)
+        U, P = U.copy(), P.copy()
+        bs, bt = np.asarray(bs, dtype=np.float64), np.asarray(bt, dtype=np.float64)
+        self._ok(self.lib.orc_nested_leapfrog(_c_int4(*dims), _ptr(bs), _ptr(bt), tau, n_outer, n_inner, _mat(U, V),
+                                              _mat(P, V)), "nested_leapfrog")
+        return U, P
 
     # ---- O11
     def leapfrog(self, dims, beta, eps, nsteps, U, P):

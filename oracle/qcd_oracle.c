@@ -604,6 +604,140 @@ int orc_leapfrog(const int L[4], double beta, double eps, int nsteps, double *U,
     return 0;
 }
 
+/* ------------------------------------------------------------------ O13 anisotropic Wilson action
+ * (PAPER.md:101 names an "anisotropic Wilson" gauge action and gives no formula; R19):
+ *   S = beta_s sum_x sum_{i<j<3} (1 - (1/3) Re tr P_ij(x)) + beta_t sum_x sum_{i<3} (1 - (1/3) Re tr P_i3(x))
+ * i.e. one coefficient for the three space-space planes and one for the three space-time planes. */
+
+static int plane_is_temporal(int mu, int nu) { return mu == 3 || nu == 3; }
+
+/* (1/3) Re tr of the space-space planes (out[0]) and of the space-time planes (out[1]) at one site */
+static void site_plaq_st(const lat_t *lat, const double *U, long s, double out[2]) {
+    out[0] = out[1] = 0;
+    for (int mu = 0; mu < 4; mu++)
+        for (int nu = mu + 1; nu < 4; nu++) {
+            cplx P[9];
+            plaq_mat(lat, U, s, mu, nu, P);
+            out[plane_is_temporal(mu, nu)] += creal(m_trace(P)) / 3.0;
+        }
+}
+
+/* avg[0] = mean over sites and the 3 space-space planes of (1/3) Re tr P, avg[1] = same over the 3 space-time
+ * planes; per_t (or NULL) is [Lt][2], a plaquette belonging to the timeslice of its base site (R13) */
+int orc_plaquette_st(const int L[4], const double *U, double avg[2], double *per_t) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !U || !avg) return 1;
+    int Lt = lat.L[3];
+    long Vs = lat.V / Lt;
+    long double tot[2] = {0, 0};
+    for (int t = 0; t < Lt; t++) {
+        long double acc[2] = {0, 0};
+        for (long s = (long)t * Vs; s < (long)(t + 1) * Vs; s++) {
+            double w[2];
+            site_plaq_st(&lat, U, s, w);
+            acc[0] += w[0];
+            acc[1] += w[1];
+        }
+        for (int k = 0; k < 2; k++) {
+            if (per_t) per_t[2 * t + k] = (double)(acc[k] / (3.0L * Vs));
+            tot[k] += acc[k];
+        }
+    }
+    for (int k = 0; k < 2; k++) avg[k] = (double)(tot[k] / (3.0L * lat.V));
+    return 0;
+}
+
+int orc_action_aniso(const int L[4], double beta_s, double beta_t, const double *U, double *S) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !U || !S) return 1;
+    long double acc = 0;
+    for (long s = 0; s < lat.V; s++) {
+        double w[2];
+        site_plaq_st(&lat, U, s, w);
+        acc += beta_s * (3.0 - w[0]) + beta_t * (3.0 - w[1]);
+    }
+    *S = (double)acc;
+    return 0;
+}
+
+/* F_mu(x) = (i/12) [ (W - W^dag) - (1/3) tr(W - W^dag) ],  W = U_mu(x) sum_{nu != mu} beta_{mu nu} (staples in nu),
+ * beta_{mu nu} = beta_t if mu or nu is the time direction, else beta_s.  Staples as in O7. */
+static void force_link_aniso(const lat_t *lat, double beta_s, double beta_t, const double *U, long s, int mu,
+                             cplx *F) {
+    cplx A[9], W[9], Wd[9], X[9];
+    m_zero(A);
+    long xpm = hop(lat, s, mu, +1);
+    for (int nu = 0; nu < 4; nu++) {
+        if (nu == mu) continue;
+        double b = plane_is_temporal(mu, nu) ? beta_t : beta_s;
+        cplx T[9], D[9];
+        long xpn = hop(lat, s, nu, +1);
+        long xmn = hop(lat, s, nu, -1);
+        long xpmmn = hop(lat, xpm, nu, -1);
+        m_dag(D, CLINK(U, xpn, mu));
+        m_mul(T, CLINK(U, xpm, nu), D);
+        m_dag(D, CLINK(U, s, nu));
+        m_mul(T, T, D);
+        for (int i = 0; i < 9; i++) A[i] += b * T[i];
+        m_dag(T, CLINK(U, xpmmn, nu));
+        m_dag(D, CLINK(U, xmn, mu));
+        m_mul(T, T, D);
+        m_mul(T, T, CLINK(U, xmn, nu));
+        for (int i = 0; i < 9; i++) A[i] += b * T[i];
+    }
+    m_mul(W, CLINK(U, s, mu), A);
+    m_dag(Wd, W);
+    for (int i = 0; i < 9; i++) X[i] = W[i] - Wd[i];
+    cplx tr3 = m_trace(X) / 3.0;
+    X[0] -= tr3;
+    X[4] -= tr3;
+    X[8] -= tr3;
+    for (int i = 0; i < 9; i++) F[i] = I * (1.0 / 12.0) * X[i];
+}
+
+int orc_gauge_force_aniso(const int L[4], int subset, double beta_s, double beta_t, const double *U, double *F) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !U || !F || subset < 0 || subset > 2) return 1;
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < lat.V; s++) {
+        if (!in_subset(&lat, s, subset)) continue;
+        for (int mu = 0; mu < 4; mu++) force_link_aniso(&lat, beta_s, beta_t, U, s, mu, LINK(F, s, mu));
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O14 two-level (multi-timescale) leapfrog
+ * ("Multi-timescale integrators were utilized", no formula; R20: Sexton-Weingarten
+ * nesting).  The action is split as S = S_1 + S_0, each an anisotropic Wilson action with coefficients
+ * (bs[k], bt[k]); S_1 is integrated with n_outer steps of eps_1 = tau/n_outer, S_0 with n_inner leapfrog
+ * steps of eps_0 = eps_1/n_inner inside every outer step:
+ *   outer step:  P += (eps_1/2) F_1;  inner leapfrog [P += (eps_0/2) F_0; n_inner x {U <- reunit(exp(i eps_0 P) U);
+ *                P += eps_0 F_0, eps_0/2 on the last}];  P += (eps_1/2) F_1
+ * written out step by step, no merging of adjacent half steps. */
+int orc_nested_leapfrog(const int L[4], const double bs[2], const double bt[2], double tau, int n_outer,
+                        int n_inner, double *U, double *P) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !U || !P || n_outer < 1 || n_inner < 1) return 1;
+    double *F = malloc(sizeof(double) * 72 * (size_t)lat.V);
+    if (!F) return 2;
+    double e1 = tau / n_outer, e0 = e1 / n_inner;
+    for (int k = 0; k < n_outer; k++) {
+        orc_gauge_force_aniso(L, 0, bs[1], bt[1], U, F);
+        orc_mom_update(L, 0, 0.5 * e1, F, P);
+        orc_gauge_force_aniso(L, 0, bs[0], bt[0], U, F);
+        orc_mom_update(L, 0, 0.5 * e0, F, P);
+        for (int j = 0; j < n_inner; j++) {
+            orc_link_update(L, 0, e0, P, U, 1);
+            orc_gauge_force_aniso(L, 0, bs[0], bt[0], U, F);
+            orc_mom_update(L, 0, j == n_inner - 1 ? 0.5 * e0 : e0, F, P);
+        }
+        orc_gauge_force_aniso(L, 0, bs[1], bt[1], U, F);
+        orc_mom_update(L, 0, 0.5 * e1, F, P);
+    }
+    free(F);
+    return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

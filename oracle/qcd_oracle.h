@@ -87,6 +87,17 @@ int orc_leapfrog(const int L[4], double beta, double eps, int nsteps, double *U,
 /* one fused MD step as the product path runs it: P += eps_p F(U); U <- reunit(exp(i eps_u P) U) */
 int orc_md_step(const int L[4], double beta, double eps_p, double eps_u, double *U, double *P);
 
+/* O13 anisotropic Wilson action (R19): beta_s on the three space-space planes, beta_t on the
+ * three space-time planes.  avg[0]/avg[1] = mean (1/3) Re tr P over space-space / space-time planes;
+ * per_t is [Lt][2] or NULL. */
+int orc_plaquette_st(const int L[4], const double *U, double avg[2], double *per_t);
+int orc_action_aniso(const int L[4], double beta_s, double beta_t, const double *U, double *S);
+int orc_gauge_force_aniso(const int L[4], int subset, double beta_s, double beta_t, const double *U, double *F);
+/* O14 two-level leapfrog (R20): level 1 (outer, n_outer steps over tau) integrates the action with
+ * coefficients (bs[1], bt[1]), level 0 (n_inner steps per outer step) the one with (bs[0], bt[0]) */
+int orc_nested_leapfrog(const int L[4], const double bs[2], const double bt[2], double tau, int n_outer,
+                        int n_inner, double *U, double *P);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus
