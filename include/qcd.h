@@ -171,6 +171,31 @@ int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, doubl
 int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,
                              void *P, void *U_work, void *stream);
 
+/* ---- anisotropic Wilson action and multi-timescale integrator ------------------
+ * The paper's demonstration ran an anisotropic Wilson gauge action with multi-timescale
+ * integrators and gives no formulas; readings R19/R20 of DESIGN.md:
+ *   S = beta_s sum_x sum_{i<j<3} (1 - (1/3) Re tr P_ij(x)) + beta_t sum_x sum_{i<3} (1 - (1/3) Re tr P_i3(x)),
+ *   F_mu(x) = (i/12)[(W - W^dag) - (1/3) tr(W - W^dag)],  W = U_mu(x) sum_{nu != mu} beta_{mu nu} staples_nu,
+ *   beta_{mu nu} = beta_t if mu or nu is the time direction (3), else beta_s.
+ * beta_s = beta_t = beta reproduces qcd_gauge_force.  Planes with coefficient 0 cost nothing. */
+int qcd_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t,
+                          const void *U, void *F, void *stream);
+/* fused P += eps * F_aniso(U) on the subset's sites */
+int qcd_force_mom_update_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t,
+                               double eps, const void *U, void *P, void *stream);
+/* out_avg[0] / out_avg[1] = mean of (1/3) Re tr P over the space-space / space-time planes (device doubles);
+ * out_per_t: device double[Lt][2] or NULL, a plaquette counted in the timeslice of its base site.
+ * S_aniso = 3 V [beta_s (1 - out_avg[0]) + beta_t (1 - out_avg[1])].  Deterministic like qcd_plaquette. */
+int qcd_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                     void *workspace, void *stream);
+/* Two-level leapfrog (Sexton-Weingarten nesting, R20) over trajectory length tau.  The action is
+ * S_1 + S_0 with coefficients (beta_s[k], beta_t[k]); level 1 takes n_outer steps of eps_1 = tau/n_outer,
+ * level 0 n_inner leapfrog steps of eps_1/n_inner inside each.  Momentum updates that act on the same links
+ * (adjacent half steps, both levels) are merged into ONE force kernel with summed plane weights, so the
+ * trajectory is 1 + n_outer*n_inner force launches and n_outer*n_inner link updates (exp + reunit). */
+int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2], const double beta_t[2],
+                        double tau, int n_outer, int n_inner, void *U, void *P, void *stream);
+
 /* Leapfrog trajectory [O11]: P += (eps/2) F; n times { U <- reunit(exp(i eps P) U); P += eps F }
  * with eps/2 on the last. */
 int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,

@@ -42,6 +42,11 @@ SIGNATURES = {
     "qcd_leapfrog": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp]),
     "qcd_md_step_single_pass": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "qcd_leapfrog_single_pass": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
+    "qcd_gauge_force_aniso": (_i, [_vp, _i, _i, _d, _d, _vp, _vp, _vp]),
+    "qcd_force_mom_update_aniso": (_i, [_vp, _i, _i, _d, _d, _d, _vp, _vp, _vp]),
+    "qcd_plaquette_st": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_nested_leapfrog": (_i, [_vp, _i, C.POINTER(C.c_double * 2), C.POINTER(C.c_double * 2), _d, _i, _i, _vp, _vp,
+                                 _vp]),
     "qcd_pack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_unpack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_get_map": (_i, [_vp, _i, _vp, _vp]),
@@ -55,7 +60,7 @@ SIGNATURES = {
 def load_library(path=LIB_PATH):
     if not os.path.exists(path):
         raise ImportError(
-            f"{path} is missing: build it with `python -m paper_1212_0785_b200.build` "
+            f"{path} is missing: build it with `python paper_1212_0785_b200/build.py` "
             "(there is no CPU fallback for the CUDA path)")
     lib = C.CDLL(path)
     for name, (res, args) in SIGNATURES.items():
@@ -194,6 +199,27 @@ def qcd_md_step_single_pass(lat, U_in, P, U_out, beta, eps_p, eps_u, stream=None
 def qcd_leapfrog_single_pass(lat, U, P, U_work, beta, eps, nsteps, stream=None):
     _check(lib.qcd_leapfrog_single_pass(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _ptr(U_work),
                                         _stream(stream)))
+
+
+def qcd_gauge_force_aniso(lat, U, F, beta_s, beta_t, subset=ALL, stream=None):
+    _check(lib.qcd_gauge_force_aniso(lat.handle, _prec(U), subset, beta_s, beta_t, _ptr(U), _ptr(F), _stream(stream)))
+
+
+def qcd_force_mom_update_aniso(lat, U, P, beta_s, beta_t, eps, subset=ALL, stream=None):
+    _check(lib.qcd_force_mom_update_aniso(lat.handle, _prec(U), subset, beta_s, beta_t, eps, _ptr(U), _ptr(P),
+                                          _stream(stream)))
+
+
+def qcd_plaquette_st(lat, U, out_avg, out_per_t, workspace, stream=None):
+    _check(lib.qcd_plaquette_st(lat.handle, _prec(U), _ptr(U), _ptr(out_avg), _ptr(out_per_t), _ptr(workspace),
+                                _stream(stream)))
+
+
+def qcd_nested_leapfrog(lat, U, P, beta_s, beta_t, tau, n_outer, n_inner, stream=None):
+    """beta_s, beta_t: (level 0 = inner, level 1 = outer)"""
+    bs, bt = (C.c_double * 2)(*beta_s), (C.c_double * 2)(*beta_t)
+    _check(lib.qcd_nested_leapfrog(lat.handle, _prec(U), C.byref(bs), C.byref(bt), tau, n_outer, n_inner, _ptr(U),
+                                   _ptr(P), _stream(stream)))
 
 
 def qcd_pack(lat, ncomp, lex_aos, dev_soa, stream=None):

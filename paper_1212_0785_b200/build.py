@@ -1,6 +1,7 @@
 """Build libqcdmd.so (the C-ABI CUDA library of include/qcd.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_1212_0785_b200.build [--force] [--verbose]
+    python paper_1212_0785_b200/build.py [--force] [--verbose]     (by path: the package itself refuses to import
+                                                                without the library it is about to build)
 
 nvcc cross-compiles without a GPU.  Objects and the ptxas resource report (registers, spills)
 go to build/; the library is written next to this file so it travels with the source tree.

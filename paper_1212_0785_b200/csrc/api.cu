@@ -287,6 +287,66 @@ int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, doub
     return launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, cur, P, true, st);
 }
 
+int qcd_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t, const void *U,
+                          void *F, void *stream) {
+    const char *fn = "qcd_gauge_force_aniso";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(F, fn));
+    QCD_TRY(check_alias(U, F, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_gauge_force_aniso(lat, prec, subset, beta_s, beta_t, 0.0, U, F, false, (cudaStream_t)stream);
+}
+
+int qcd_force_mom_update_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t,
+                               double eps, const void *U, void *P, void *stream) {
+    const char *fn = "qcd_force_mom_update_aniso";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    return launch_gauge_force_aniso(lat, prec, subset, beta_s, beta_t, eps, U, P, true, (cudaStream_t)stream);
+}
+
+int qcd_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                     void *workspace, void *stream) {
+    const char *fn = "qcd_plaquette_st";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    if (!out_avg || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    return launch_plaquette_st(lat, prec, U, out_avg, out_per_t, (double *)workspace, (cudaStream_t)stream);
+}
+
+int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2], const double beta_t[2], double tau,
+                        int n_outer, int n_inner, void *U, void *P, void *stream) {
+    const char *fn = "qcd_nested_leapfrog";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    if (!beta_s || !beta_t) return bad(QCD_EINVAL, "%s: NULL coefficient array", fn);
+    if (n_outer < 1 || n_inner < 1) return bad(QCD_EINVAL, "%s: step counts must be >= 1", fn);
+    cudaStream_t st = (cudaStream_t)stream;
+    const double e1 = tau / n_outer, e0 = e1 / n_inner;
+    // a momentum update with step a0 of level 0 and a1 of level 1 at fixed U is one force kernel with plane
+    // weights a0*beta[0] + a1*beta[1] and eps = 1
+    auto kick = [&](double a0, double a1) {
+        return launch_gauge_force_aniso(lat, prec, QCD_ALL, a0 * beta_s[0] + a1 * beta_s[1],
+                                        a0 * beta_t[0] + a1 * beta_t[1], 1.0, U, P, true, st);
+    };
+    QCD_TRY(kick(0.5 * e0, 0.5 * e1));
+    for (int k = 0; k < n_outer; k++)
+        for (int j = 0; j < n_inner; j++) {
+            QCD_TRY(launch_link_update(lat, prec, QCD_ALL, e0, P, U, 1, st));
+            const bool inner_end = j == n_inner - 1, traj_end = inner_end && k == n_outer - 1;
+            if (!inner_end) QCD_TRY(kick(e0, 0.0));
+            else if (!traj_end) QCD_TRY(kick(e0, e1));  // (e0/2 + e1/2) closing this outer step + the same opening the next
+            else QCD_TRY(kick(0.5 * e0, 0.5 * e1));
+        }
+    return QCD_OK;
+}
+
 int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream) {
     const char *fn = "qcd_pack";
     QCD_TRY(check_common(lat, prec, fn));

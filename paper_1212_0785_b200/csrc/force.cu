@@ -54,11 +54,15 @@ __device__ __forceinline__ void ldU(M3<T> &m, const pair_t<T> *__restrict__ f, i
     else load_link(m, f, V, mu, cb);
 }
 
-template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1, bool REC = false>
+// ANISO (R19; "anisotropic Wilson" action): the staples of plane (mu,nu) carry the weight
+// wt if mu or nu is the time direction, else ws (c is then 1/12); planes of weight zero are skipped, which
+// is what the levels of the multi-timescale integrator (space-space planes only / space-time planes only) use.
+template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1, bool REC = false,
+          bool ANISO = false>
 __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out, const T eps_u,
-                                                    pair_t<T> *__restrict__ Uout) {
+                                                    pair_t<T> *__restrict__ Uout, const T ws, const T wt) {
     const Site st = tile_site(lat, tile, threadIdx.x);
     const int V = lat.V;
     const int par = st.par;
@@ -82,6 +86,8 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
 #pragma unroll
         for (int k = 1; k < 4; k++) {
             const int nu = (mu + k) & 3;
+            const T w = ANISO ? ((mu == 3 || nu == 3) ? wt : ws) : T(1);
+            if (ANISO && w == T(0)) continue;  // warp-uniform
             const int dfn = nu == 0 ? df[0] : nu == 1 ? df[1] : nu == 2 ? df[2] : df[3];
             const int dbn = nu == 0 ? db[0] : nu == 1 ? db[1] : nu == 2 ? db[2] : db[3];
             const int cb_pn = cb_of(lat, st.s + dfn, par ^ 1);      // x + nu
@@ -92,12 +98,14 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
             ldU<REC>(X, U, V, nu, cb_pm);
             ldU<REC>(Y, U, V, mu, cb_pn);
             mul<false, true, false>(Z, X, Y);
+            if (ANISO) scale(Z, w);
             ldU<REC>(X, U, V, nu, cb);
             mul<false, true, true>(A, Z, X);
             // down staple: U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu)
             ldU<REC>(X, U, V, nu, cb_pmmn);
             ldU<REC>(Y, U, V, mu, cb_mn);
             mul<true, true, false>(Z, X, Y);
+            if (ANISO) scale(Z, w);
             ldU<REC>(X, U, V, nu, cb_mn);
             mul<false, false, true>(A, Z, X);
         }
@@ -497,9 +505,9 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
         const TileP tp = choose_tile(lat->p, subset, 128);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         if (getenv("QCD_SU3_REC"))  // sweep knob: SU(3) links only (two-row loads); measured no gain, off by default
-            force_kernel<T, FUSED, false, false, 128, 3, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+            force_kernel<T, FUSED, false, false, 128, 3, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         else
-            force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+            force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         return;
     }
     if (!strcmp(v, "site256")) {  // 256-thread blocks, one per SM in fp64 (254 registers), momenta loaded early
@@ -507,9 +515,9 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         const char *pm = getenv("QCD_EARLY_P");  // sweep knob; default on
         if (!pm || atoi(pm))
-            force_kernel<T, FUSED, true, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+            force_kernel<T, FUSED, true, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         else
-            force_kernel<T, FUSED, false, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr);
+            force_kernel<T, FUSED, false, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         return;
     }
     if (!strcmp(v, "plane")) {
@@ -542,6 +550,28 @@ static int launch_force_t(const qcd_lattice *lat, int subset, double beta, doubl
     return check_launch(fused ? "force_mom_update" : "gauge_force");
 }
 
+// Anisotropic force (plane weights ws, wt; eps = 1 folds a step size into the weights)
+template <typename T>
+static int launch_force_aniso_t(const qcd_lattice *lat, int subset, double ws, double wt, double eps, const void *U,
+                                void *out, bool fused, cudaStream_t st) {
+    const TileP tp = choose_tile(lat->p, subset, 128);
+    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+    const T c = (T)(1.0 / 12.0);
+    if (fused)
+        force_kernel<T, true, false, false, 128, 3, false, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(
+            lat->p, tp, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, T(0), nullptr, (T)ws, (T)wt);
+    else
+        force_kernel<T, false, false, false, 128, 3, false, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(
+            lat->p, tp, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, T(0), nullptr, (T)ws, (T)wt);
+    return check_launch(fused ? "force_mom_update_aniso" : "gauge_force_aniso");
+}
+
+int launch_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double ws, double wt, double eps,
+                             const void *U, void *out, bool fused_mom, cudaStream_t st) {
+    return prec == QCD_F64 ? launch_force_aniso_t<double>(lat, subset, ws, wt, eps, U, out, fused_mom, st)
+                           : launch_force_aniso_t<float>(lat, subset, ws, wt, eps, U, out, fused_mom, st);
+}
+
 // Single-pass MD step: P += eps_p F(U); Uout = reunit(exp(i eps_u P) U).  Subset ALL only (every link moves).
 template <typename T>
 static int launch_md_single_t(const qcd_lattice *lat, double beta, double eps_p, double eps_u, const void *U, void *P,
@@ -549,7 +579,7 @@ static int launch_md_single_t(const qcd_lattice *lat, double beta, double eps_p,
     const TileP tp = choose_tile(lat->p, QCD_ALL, 128);
     const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
     force_kernel<T, true, false, true, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(
-        lat->p, tp, (T)(beta / 12.0), (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u, (pair_t<T> *)Uout);
+        lat->p, tp, (T)(beta / 12.0), (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u, (pair_t<T> *)Uout, T(0), T(0));
     return check_launch("md_step_single_pass");
 }
 

@@ -53,6 +53,13 @@ int check_launch(const char *what);
 // kernel launchers, one per translation unit; prec already validated. All return QCD_OK/QCD_ECUDA.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
                        void *out, bool fused_mom, cudaStream_t st);
+// anisotropic Wilson force (force.cu): staples of space-space planes weighted ws, space-time planes wt
+// (weights include beta; eps multiplies F in the fused momentum update)
+int launch_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double ws, double wt, double eps,
+                             const void *U, void *out, bool fused_mom, cudaStream_t st);
+// space-space / space-time plaquette averages (reduce.cu): out_avg[2], out_per_t[Lt][2] or NULL
+int launch_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                        double *ws, cudaStream_t st);
 // single-pass MD step (force.cu): P += eps_p F(U); Uout = reunit(exp(i eps_u P) U); U and Uout distinct
 int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
                      void *Uout, cudaStream_t st);

@@ -31,8 +31,10 @@ __device__ __forceinline__ double block_sum(double v) {
 // ---- per-site values -----------------------------------------------------------------------
 
 // sum_{mu<nu} Re tr P_mu_nu(x), P_mu_nu(x) = [U_mu(x) U_nu(x+mu)] [U_nu(x) U_mu(x+nu)]^dagger
+// which: 0 = all six planes, 1 = the three space-space planes, 2 = the three space-time planes (R19)
 template <typename T>
-__device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T> *__restrict__ U, int cb) {
+__device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T> *__restrict__ U, int cb,
+                                                 int which = 0) {
     const Site st = site_of_cb(lat, cb);
     const int V = lat.V;
     int cbf[4];
@@ -45,6 +47,7 @@ __device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T
         load_link(Um, U, V, mu, cb);
 #pragma unroll
         for (int nu = mu + 1; nu < 4; nu++) {
+            if ((which == 1 && nu == 3) || (which == 2 && nu != 3)) continue;
             M3<T> A, X, Y;
             load_link(A, U, V, nu, cbf[mu]);
             mul<false, false, false>(X, Um, A);
@@ -82,7 +85,8 @@ __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int 
 
 // ---- pass 1 --------------------------------------------------------------------------------
 
-// grid (chunks_per_seg, nseg, ncomp_out); kind < 0: plaquette.
+// grid (chunks_per_seg, nseg, ncomp_out); kind = -1: plaquette; kind = -2: comp 0 = space-space planes,
+// comp 1 = space-time planes.
 // partial[(comp*nseg + seg)*cps + chunk], seg = 2*t + parity
 template <typename T>
 __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, const int kind, const int ncomp,
@@ -97,7 +101,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, cons
         const int i = blockIdx.x * RED_CHUNK + k * RED_THREADS + threadIdx.x;
         if (i < Vsh) {
             const int cb = seg_begin + i;
-            acc += kind < 0 ? site_plaquette<T>(lat, (const pair_t<T> *)field, cb)
+            acc += kind < 0 ? site_plaquette<T>(lat, (const pair_t<T> *)field, cb, kind == -1 ? 0 : 1 + comp)
                             : site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb);
         }
     }
@@ -178,6 +182,26 @@ int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *ou
                      cudaStream_t st) {
     return prec == QCD_F64 ? plaquette_t<double>(lat, U, out_avg, out_per_t, ws, st)
                            : plaquette_t<float>(lat, U, out_avg, out_per_t, ws, st);
+}
+
+template <typename T>
+static int plaquette_st_t(const qcd_lattice *lat, const void *U, double *out_avg, double *out_per_t, double *ws,
+                          cudaStream_t st) {
+    const LatP &p = lat->p;
+    const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
+    reduce_pass1<T><<<dim3(cps, nseg, 2), RED_THREADS, 0, st>>>(p, -2, 72, U, ws);
+    const int Lt = p.L[3];
+    const double Vs = (double)(p.V / Lt);
+    if (out_per_t)  // out_per_t[t*2 + comp]
+        reduce_pass2<<<dim3(Lt, 2), RED_THREADS, 0, st>>>(ws, Lt, 2 * cps, 1.0 / (9.0 * Vs), out_per_t, 2);
+    reduce_pass2_global<<<2, RED_THREADS, 0, st>>>(ws, nseg, cps, 2, 1.0 / (9.0 * (double)p.V), out_avg);
+    return check_launch("plaquette_st");
+}
+
+int launch_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                        double *ws, cudaStream_t st) {
+    return prec == QCD_F64 ? plaquette_st_t<double>(lat, U, out_avg, out_per_t, ws, st)
+                           : plaquette_st_t<float>(lat, U, out_avg, out_per_t, ws, st);
 }
 
 template <typename T>

@@ -150,6 +150,15 @@ __device__ __forceinline__ void zero(M3<T> &A) {
     for (int e = 0; e < 9; e++) A.re[e] = A.im[e] = T(0);
 }
 
+template <typename T>
+__device__ __forceinline__ void scale(M3<T> &A, T w) {
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+        A.re[e] *= w;
+        A.im[e] *= w;
+    }
+}
+
 // ---- projection (O7): F = (i c)[(W - W^dag) - (1/3) tr(W - W^dag)], c = beta/12.
 // W - W^dag =: X is anti-Hermitian: X_ii = 2i Im W_ii, X_ij = W_ij - conj(W_ji).
 // i*X is Hermitian; F_ii = -2c (Im W_ii - mean Im W_kk), F_ij = i c (W_ij - conj(W_ji)).
