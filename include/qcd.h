@@ -196,6 +196,26 @@ int qcd_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *ou
 int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2], const double beta_t[2],
                         double tau, int n_outer, int n_inner, void *U, void *P, void *stream);
 
+/* ---- launch-parameter database of the auto-tuner (section 4) -------
+ * The paper times every kernel as a function of the threads per block N_t and stores the best value in a
+ * database.  Here the measuring lives in paper_1212_0785_b200/autotune.py (it calls the public kernels);
+ * these calls are the database the launchers consult.  Key: (lattice extents, prec, subset ALL or
+ * EVEN/ODD, kernel).  Value: for QCD_KERNEL_FORCE a kernel variant and a 4-D block tile (tile[0] = 0 or
+ * tile = NULL: the library's own choice; extents must divide the lattice, tile[0] even, and the block must
+ * not exceed the variant's thread limit: 128 sites for SITE, 256 for SITE256/PIPE/PLANE, 128 for LINK);
+ * for QCD_KERNEL_LINK_UPDATE / QCD_KERNEL_MOM_UPDATE the threads per block (multiple of 32, 32..256).
+ * Environment variables QCD_FORCE_VARIANT / QCD_TILE, when set, still win (sweeps).  Results never depend
+ * on these settings beyond rounding order; reductions are not tunable (fixed geometry, determinism).
+ * Host-only, thread-safe, process-global.  qcd_tune_get returns QCD_EINVAL when no entry exists. */
+enum { QCD_KERNEL_FORCE = 0, QCD_KERNEL_LINK_UPDATE = 1, QCD_KERNEL_MOM_UPDATE = 2 };
+enum { QCD_FORCE_SITE = 0, QCD_FORCE_SITE256 = 1, QCD_FORCE_PIPE = 2, QCD_FORCE_PLANE = 3, QCD_FORCE_LINK = 4,
+       QCD_FORCE_TILE = 5, QCD_FORCE_PLAQ = 6 };
+int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int variant, const int tile[4],
+                 int threads);
+int qcd_tune_get(const qcd_lattice *lat, int prec, int subset, int kernel, int *variant, int tile[4],
+                 int *threads);
+int qcd_tune_clear(void);
+
 /* Leapfrog trajectory [O11]: P += (eps/2) F; n times { U <- reunit(exp(i eps P) U); P += eps F }
  * with eps/2 on the last. */
 int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,

@@ -16,6 +16,8 @@ F32, F64 = 0, 1
 ALL, EVEN, ODD = 0, 1, 2
 SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
 OK, EINVAL, EDIMS, EALIGN, EALIAS, EWORKSPACE, ECUDA = range(7)
+KERNEL_FORCE, KERNEL_LINK_UPDATE, KERNEL_MOM_UPDATE = 0, 1, 2
+FORCE_VARIANTS = ("site", "site256", "pipe", "plane", "link", "tile", "plaq")  # index = QCD_FORCE_* value
 MAP_CB_OF_LEX, MAP_LEX_OF_CB, MAP_NBR_FWD0, MAP_NBR_BWD0, MAP_PARITY, MAP_TSLICE = 0, 1, 2, 6, 10, 11
 
 # every symbol include/qcd.h declares, with its ctypes signature (restype, argtypes)
@@ -47,6 +49,9 @@ SIGNATURES = {
     "qcd_plaquette_st": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
     "qcd_nested_leapfrog": (_i, [_vp, _i, C.POINTER(C.c_double * 2), C.POINTER(C.c_double * 2), _d, _i, _i, _vp, _vp,
                                  _vp]),
+    "qcd_tune_set": (_i, [_vp, _i, _i, _i, _i, C.POINTER(C.c_int * 4), _i]),
+    "qcd_tune_get": (_i, [_vp, _i, _i, _i, C.POINTER(_i), C.POINTER(C.c_int * 4), C.POINTER(_i)]),
+    "qcd_tune_clear": (_i, []),
     "qcd_pack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_unpack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
     "qcd_get_map": (_i, [_vp, _i, _vp, _vp]),
@@ -220,6 +225,22 @@ def qcd_nested_leapfrog(lat, U, P, beta_s, beta_t, tau, n_outer, n_inner, stream
     bs, bt = (C.c_double * 2)(*beta_s), (C.c_double * 2)(*beta_t)
     _check(lib.qcd_nested_leapfrog(lat.handle, _prec(U), C.byref(bs), C.byref(bt), tau, n_outer, n_inner, _ptr(U),
                                    _ptr(P), _stream(stream)))
+
+
+def qcd_tune_set(lat, prec, subset, kernel, variant=0, tile=None, threads=0):
+    arr = (C.c_int * 4)(*tile) if tile else None
+    _check(lib.qcd_tune_set(lat.handle, prec, subset, kernel, variant, C.byref(arr) if tile else None, threads))
+
+
+def qcd_tune_get(lat, prec, subset, kernel):
+    """(variant, tile, threads) or None when the database has no entry"""
+    v, t, arr = _i(), _i(), (C.c_int * 4)()
+    rc = lib.qcd_tune_get(lat.handle, prec, subset, kernel, C.byref(v), C.byref(arr), C.byref(t))
+    return None if rc != OK else (v.value, tuple(arr), t.value)
+
+
+def qcd_tune_clear():
+    _check(lib.qcd_tune_clear())
 
 
 def qcd_pack(lat, ncomp, lex_aos, dev_soa, stream=None):

@@ -347,6 +347,56 @@ int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2]
     return QCD_OK;
 }
 
+int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int variant, const int tile[4],
+                 int threads) {
+    const char *fn = "qcd_tune_set";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    TuneCfg cfg = {0, {0, 0, 0, 0}, 0};
+    if (kernel == QCD_KERNEL_FORCE) {
+        if (variant < QCD_FORCE_SITE || variant > QCD_FORCE_PLAQ) return bad(QCD_EINVAL, "%s: unknown force variant", fn);
+        cfg.variant = variant;
+        if (tile && tile[0]) {
+            long sites = 1;
+            for (int d = 0; d < 4; d++) {
+                if (tile[d] < 1 || lat->p.L[d] % tile[d]) return bad(QCD_EINVAL, "%s: tile must divide the lattice", fn);
+                sites *= tile[d];
+                cfg.tile[d] = tile[d];
+            }
+            if (tile[0] & 1) return bad(QCD_EINVAL, "%s: tile[0] must be even", fn);
+            const long threads_needed = subset == QCD_ALL ? sites : sites / 2;
+            const long limit = variant == QCD_FORCE_SITE || variant == QCD_FORCE_LINK ? 128 : 256;
+            if (variant <= QCD_FORCE_LINK && threads_needed > limit)
+                return bad(QCD_EINVAL, "%s: tile has more sites than the variant's block can hold", fn);
+        }
+    } else if (kernel == QCD_KERNEL_LINK_UPDATE || kernel == QCD_KERNEL_MOM_UPDATE) {
+        if (threads < 32 || threads > 256 || threads % 32) return bad(QCD_EINVAL, "%s: threads must be 32..256, multiple of 32", fn);
+        cfg.threads = threads;
+    } else {
+        return bad(QCD_EINVAL, "%s: unknown kernel", fn);
+    }
+    tune_store(lat, prec, subset, kernel, cfg);
+    return QCD_OK;
+}
+
+int qcd_tune_get(const qcd_lattice *lat, int prec, int subset, int kernel, int *variant, int tile[4], int *threads) {
+    const char *fn = "qcd_tune_get";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    TuneCfg cfg;
+    if (!tune_lookup(lat, prec, subset, kernel, cfg)) return bad(QCD_EINVAL, "%s: no entry", fn);
+    if (variant) *variant = cfg.variant;
+    if (tile)
+        for (int d = 0; d < 4; d++) tile[d] = cfg.tile[d];
+    if (threads) *threads = cfg.threads;
+    return QCD_OK;
+}
+
+int qcd_tune_clear(void) {
+    tune_clear_all();
+    return QCD_OK;
+}
+
 int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream) {
     const char *fn = "qcd_pack";
     QCD_TRY(check_common(lat, prec, fn));

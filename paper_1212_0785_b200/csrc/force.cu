@@ -444,7 +444,7 @@ static int divisors(int n, bool even, int *out) {
 // as possible (never above it), preferring a long x extent (coalescing: T0/2 consecutive sites are
 // contiguous in memory) and then the smallest surface (L1 reuse of neighbour links).
 // QCD_TILE="tx,ty,tz,tt" overrides for block-shape sweeps (the paper's N_t tuning).
-static TileP choose_tile(const LatP &lat, int subset, int target) {
+static TileP choose_tile(const LatP &lat, int subset, int target, const int *tuned = nullptr) {
     TileP tp;
     tp.npar = subset == QCD_ALL ? 2 : 1;
     tp.par0 = subset == QCD_ODD ? 1 : 0;
@@ -452,7 +452,13 @@ static TileP choose_tile(const LatP &lat, int subset, int target) {
     const char *env = getenv("QCD_TILE");
     int e[4];
     bool have = false;
-    if (env && sscanf(env, "%d,%d,%d,%d", &e[0], &e[1], &e[2], &e[3]) == 4) {
+    // the environment (sweeps) wins over the tuner's database entry, which wins over the heuristic below
+    bool given = env && sscanf(env, "%d,%d,%d,%d", &e[0], &e[1], &e[2], &e[3]) == 4;
+    if (!given && tuned && tuned[0]) {
+        memcpy(e, tuned, sizeof e);
+        given = true;
+    }
+    if (given) {
         have = true;
         for (int d = 0; d < 4; d++)
             if (e[d] < 1 || lat.L[d] % e[d]) have = false;
@@ -495,14 +501,38 @@ static TileP choose_tile(const LatP &lat, int subset, int target) {
 // PAPER.md:57): "site" (default) = one thread per site, 128-thread blocks; "site256" = the same kernel in
 // 256-thread blocks with the momenta loaded early; "pipe" / "plane" = the hand-pipelined and the plane-wise
 // kernels above; "link" = one thread per (site, mu) with QCD_FORCE_THREADS in {256, 512} threads per block.
-template <typename T, bool FUSED>
-static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const pair_t<T> *U, pair_t<T> *out,
-                           cudaStream_t st) {
+// kernel variant and tile for this launch: QCD_FORCE_VARIANT (sweeps) > tuner database (tune.cu) > default
+struct ForceSel {
+    int variant;
+    int tile[4];
+};
+static const char *const kVariantNames[] = {"site", "site256", "pipe", "plane", "link", "tile", "plaq"};
+
+static ForceSel force_sel(const qcd_lattice *lat, int prec, int subset) {
+    ForceSel fs = {QCD_FORCE_SITE, {0, 0, 0, 0}};
+    TuneCfg cfg;
+    if (tune_lookup(lat, prec, subset, QCD_KERNEL_FORCE, cfg)) {
+        fs.variant = cfg.variant;
+        memcpy(fs.tile, cfg.tile, sizeof fs.tile);
+    }
     const char *v = getenv("QCD_FORCE_VARIANT");
-    if (!v || strcmp(v, "site256") && strcmp(v, "plane") && strcmp(v, "pipe") && strcmp(v, "link")) {
+    if (v) {
+        fs.variant = QCD_FORCE_SITE;
+        for (int k = 0; k <= QCD_FORCE_PLAQ; k++)
+            if (!strcmp(v, kVariantNames[k])) fs.variant = k;
+    }
+    return fs;
+}
+
+template <typename T, bool FUSED>
+static void launch_force_v(const qcd_lattice *lat, int subset, const ForceSel &fs, T c, T eps, const pair_t<T> *U,
+                           pair_t<T> *out, cudaStream_t st) {
+    const int *tuned = fs.tile;
+    const int var = fs.variant;
+    if (var != QCD_FORCE_SITE256 && var != QCD_FORCE_PLANE && var != QCD_FORCE_PIPE && var != QCD_FORCE_LINK) {
         // default: 128-thread blocks, three per SM (168 registers in fp64, 12 warps/SM); measured best at
         // 32^3x64 in both precisions (profiles/r01c_force_sweeps.md)
-        const TileP tp = choose_tile(lat->p, subset, 128);
+        const TileP tp = choose_tile(lat->p, subset, 128, tuned);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         if (getenv("QCD_SU3_REC"))  // sweep knob: SU(3) links only (two-row loads); measured no gain, off by default
             force_kernel<T, FUSED, false, false, 128, 3, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
@@ -510,8 +540,8 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
             force_kernel<T, FUSED, false, false, 128, 3><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         return;
     }
-    if (!strcmp(v, "site256")) {  // 256-thread blocks, one per SM in fp64 (254 registers), momenta loaded early
-        const TileP tp = choose_tile(lat->p, subset, 256);
+    if (var == QCD_FORCE_SITE256) {  // 256-thread blocks, one per SM in fp64 (254 registers), momenta loaded early
+        const TileP tp = choose_tile(lat->p, subset, 256, tuned);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         const char *pm = getenv("QCD_EARLY_P");  // sweep knob; default on
         if (!pm || atoi(pm))
@@ -520,21 +550,21 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
             force_kernel<T, FUSED, false, false><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out, T(0), nullptr, T(0), T(0));
         return;
     }
-    if (!strcmp(v, "plane")) {
-        const TileP tp = choose_tile(lat->p, subset, 256);
+    if (var == QCD_FORCE_PLANE) {
+        const TileP tp = choose_tile(lat->p, subset, 256, tuned);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         force_plane_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
         return;
     }
-    if (!strcmp(v, "pipe")) {
-        const TileP tp = choose_tile(lat->p, subset, 256);
+    if (var == QCD_FORCE_PIPE) {
+        const TileP tp = choose_tile(lat->p, subset, 256, tuned);
         const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
         force_pipe_kernel<T, FUSED><<<blocks, tp.tsp * tp.npar, 0, st>>>(lat->p, tp, c, eps, U, out);
         return;
     }
     const char *t = getenv("QCD_FORCE_THREADS");
     const int nt = t ? atoi(t) : 512;
-    const TileP tp = choose_tile(lat->p, subset, nt == 256 ? 64 : 128);
+    const TileP tp = choose_tile(lat->p, subset, nt == 256 ? 64 : 128, tuned);
     const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
     const int threads = 4 * tp.tsp * tp.npar;
     if (nt == 256) force_link_kernel<T, FUSED, 256><<<blocks, threads, 0, st>>>(lat->p, tp, c, eps, U, out);
@@ -542,11 +572,11 @@ static void launch_force_v(const qcd_lattice *lat, int subset, T c, T eps, const
 }
 
 template <typename T>
-static int launch_force_t(const qcd_lattice *lat, int subset, double beta, double eps, const void *U, void *out,
-                          bool fused, cudaStream_t st) {
+static int launch_force_t(const qcd_lattice *lat, int subset, const ForceSel &fs, double beta, double eps,
+                          const void *U, void *out, bool fused, cudaStream_t st) {
     const T c = (T)(beta / 12.0);
-    if (fused) launch_force_v<T, true>(lat, subset, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
-    else launch_force_v<T, false>(lat, subset, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
+    if (fused) launch_force_v<T, true>(lat, subset, fs, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
+    else launch_force_v<T, false>(lat, subset, fs, c, (T)eps, (const pair_t<T> *)U, (pair_t<T> *)out, st);
     return check_launch(fused ? "force_mom_update" : "gauge_force");
 }
 
@@ -595,15 +625,15 @@ int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p
 // (force_plaq.cu, needs unitary links) exist for subset ALL only.  DESIGN.md section 6 has the measurements.
 int launch_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
                        void *out, bool fused_mom, cudaStream_t st) {
-    const char *v = getenv("QCD_FORCE_VARIANT");
-    if (subset == QCD_ALL && v && !strcmp(v, "plaq"))
+    const ForceSel fs = force_sel(lat, prec, subset);
+    if (subset == QCD_ALL && fs.variant == QCD_FORCE_PLAQ)
         return launch_gauge_force_plaq(lat, prec, beta, eps, U, out, fused_mom, st);
-    if (subset == QCD_ALL && v && !strcmp(v, "tile")) {
+    if (subset == QCD_ALL && fs.variant == QCD_FORCE_TILE) {
         const int rc = launch_gauge_force_tile(lat, prec, beta, eps, U, out, fused_mom, st);
         if (rc >= 0) return rc;
     }
-    return prec == QCD_F64 ? launch_force_t<double>(lat, subset, beta, eps, U, out, fused_mom, st)
-                           : launch_force_t<float>(lat, subset, beta, eps, U, out, fused_mom, st);
+    return prec == QCD_F64 ? launch_force_t<double>(lat, subset, fs, beta, eps, U, out, fused_mom, st)
+                           : launch_force_t<float>(lat, subset, fs, beta, eps, U, out, fused_mom, st);
 }
 
 }  // namespace qcd

@@ -47,6 +47,16 @@ struct qcd_lattice {
 
 namespace qcd {
 
+// one entry of the auto-tuner's database (tune.cu)
+struct TuneCfg {
+    int variant;   // QCD_FORCE_* for the stencil kernel, ignored otherwise
+    int tile[4];   // 4-D block tile of the stencil kernel; tile[0] == 0: library's own choice
+    int threads;   // threads per block of a site-local kernel; 0: library default
+};
+bool tune_lookup(const qcd_lattice *lat, int prec, int subset, int kernel, TuneCfg &out);
+void tune_store(const qcd_lattice *lat, int prec, int subset, int kernel, const TuneCfg &cfg);
+void tune_clear_all();
+
 void set_error(const char *fmt, ...);
 int check_launch(const char *what);
 

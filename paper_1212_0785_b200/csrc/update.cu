@@ -54,12 +54,18 @@ __global__ void __launch_bounds__(256) mom_update_kernel(const int V, const int 
     }
 }
 
+// threads per block N_t: the tuner's database entry or the default
+static int tuned_threads(const qcd_lattice *lat, int prec, int subset, int kernel, int dflt) {
+    TuneCfg cfg;
+    return tune_lookup(lat, prec, subset, kernel, cfg) && cfg.threads ? cfg.threads : dflt;
+}
+
 template <typename T>
 static int launch_link_update_t(const qcd_lattice *lat, int subset, double eps, const void *P, void *U, int mode,
                                 cudaStream_t st) {
     int begin, count;
     subset_range(lat->p, subset, begin, count);
-    const int threads = 128;
+    const int threads = tuned_threads(lat, sizeof(T) == 8 ? QCD_F64 : QCD_F32, subset, QCD_KERNEL_LINK_UPDATE, 128);
     const dim3 grid((count + threads - 1) / threads, 4);
     const pair_t<T> *p = (const pair_t<T> *)P;
     pair_t<T> *u = (pair_t<T> *)U;
@@ -80,7 +86,7 @@ static int launch_mom_update_t(const qcd_lattice *lat, int subset, double eps, c
                                cudaStream_t st) {
     int begin, count;
     subset_range(lat->p, subset, begin, count);
-    const int threads = 256;
+    const int threads = tuned_threads(lat, sizeof(T) == 8 ? QCD_F64 : QCD_F32, subset, QCD_KERNEL_MOM_UPDATE, 256);
     const dim3 grid((count + threads - 1) / threads, 4);
     mom_update_kernel<T><<<grid, threads, 0, st>>>(lat->p.V, begin, count, (T)eps, (const pair_t<T> *)F,
                                                    (pair_t<T> *)P);

@@ -100,3 +100,28 @@ def test_product_path_does_not_import_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1212_0785_b200" not in text and "from paper_1212_0785_b200" not in text
             assert "csrc/" not in text or "shares no code" in text
+
+
+def test_tuning_database_roundtrip_and_validation():
+    """qcd_tune_set / qcd_tune_get / qcd_tune_clear are host-only (the N_t database)"""
+    from paper_1212_0785_b200 import binding as qcd
+    qcd.qcd_tune_clear()
+    lat, other = qcd.Lattice((8, 8, 8, 16)), qcd.Lattice((8, 8, 8, 4))
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) is None
+    qcd.qcd_tune_set(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index("site256"), (8, 4, 4, 2))
+    qcd.qcd_tune_set(lat, qcd.F64, qcd.EVEN, qcd.KERNEL_LINK_UPDATE, threads=64)
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) == (1, (8, 4, 4, 2), 0)
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ODD, qcd.KERNEL_LINK_UPDATE) == (0, (0, 0, 0, 0), 64)  # EVEN/ODD share
+    assert qcd.qcd_tune_get(lat, qcd.F32, qcd.ALL, qcd.KERNEL_FORCE) is None  # keyed on precision
+    assert qcd.qcd_tune_get(other, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) is None  # and on the extents
+    qcd.qcd_tune_set(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE, 0, None)  # overwrite: library's own tile
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) == (0, (0, 0, 0, 0), 0)
+    for bad in [dict(kernel=qcd.KERNEL_FORCE, variant=9), dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(3, 2, 2, 2)),
+                dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(8, 8, 8, 2)),  # 1024 sites > 128-thread block
+                dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(5, 2, 2, 2)), dict(kernel=qcd.KERNEL_MOM_UPDATE, threads=48),
+                dict(kernel=qcd.KERNEL_LINK_UPDATE, threads=512), dict(kernel=7, threads=64)]:
+        with pytest.raises(qcd.QcdError) as e:
+            qcd.qcd_tune_set(lat, qcd.F64, qcd.ALL, **bad)
+        assert e.value.code == qcd.EINVAL
+    qcd.qcd_tune_clear()
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.EVEN, qcd.KERNEL_LINK_UPDATE) is None
