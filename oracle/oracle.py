@@ -58,6 +58,9 @@ class Oracle:
         L.orc_hamiltonian.argtypes = [_c_int4, C.c_double, _dp, _dp, _dp, _dp]
         L.orc_leapfrog.argtypes = [_c_int4, C.c_double, C.c_double, C.c_int, _dp, _dp]
         L.orc_md_step.argtypes = [_c_int4, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_spinor_gaussian.argtypes = [_c_int4, C.c_int, C.c_uint64, C.c_uint32, _dp]
+        L.orc_inner_product.argtypes = [_c_int4, C.c_int, C.c_int, _dp, _dp, _dp]
+        L.orc_inner_product_multi.argtypes = [_c_int4, C.c_int, _dp, _dp, _dp]
         L.orc_plaquette_st.argtypes = [_c_int4, _dp, _dp, _dp]
         L.orc_action_aniso.argtypes = [_c_int4, C.c_double, C.c_double, _dp, _dp]
         L.orc_gauge_force_aniso.argtypes = [_c_int4, C.c_int, C.c_double, C.c_double, _dp, _dp]
@@ -267,6 +270,24 @@ class Oracle:
         self._ok(self.lib.orc_nested_leapfrog(_c_int4(*dims), _ptr(bs), _ptr(bt), tau, n_outer, n_inner, _mat(U, V),
                                               _mat(P, V)), "nested_leapfrog")
         return U, P
+
+    # ---- O15 / O16 spin-colour vectors: complex128[V, 12]
+    def spinor_gaussian(self, dims, seed, stream_id=0, subset=ALL, out=None):
+        eta = np.zeros((self.volume(dims), 12), dtype=np.complex128) if out is None else out
+        self._ok(self.lib.orc_spinor_gaussian(_c_int4(*dims), subset, seed, stream_id, _ptr(eta)), "spinor_gaussian")
+        return eta
+
+    def inner_product(self, dims, a, b, subset=ALL):
+        assert a.dtype == b.dtype == np.complex128 and a.shape == b.shape and a.flags.c_contiguous and b.flags.c_contiguous
+        out = np.empty(2)
+        self._ok(self.lib.orc_inner_product(_c_int4(*dims), subset, a.shape[1], _ptr(a), _ptr(b), _ptr(out)), "inner")
+        return complex(out[0], out[1])
+
+    def inner_product_multi(self, dims, a, b):
+        assert a.dtype == b.dtype == np.complex128 and a.shape == b.shape and a.flags.c_contiguous and b.flags.c_contiguous
+        out = np.empty((dims[3], 2))
+        self._ok(self.lib.orc_inner_product_multi(_c_int4(*dims), a.shape[1], _ptr(a), _ptr(b), _ptr(out)), "inner_multi")
+        return out[:, 0] + 1j * out[:, 1]
 
     # ---- O11
     def leapfrog(self, dims, beta, eps, nsteps, U, P):

@@ -738,6 +738,70 @@ int orc_nested_leapfrog(const int L[4], const double bs[2], const double bt[2], 
     return 0;
 }
 
+/* ------------------------------------------------------------------ O15 / O16 pseudofermion-side site operations
+ * ("a pseudofermion refresh"; only the site-parallel pieces outside the Dirac operator: the
+ * Gaussian fill of a spin-colour vector field and the norm / inner-product reductions; R21).
+ * A spin-colour vector has 4 spins x 3 colours = 12 complex components per site, canonical layout
+ * double[V][12][2] with component k = 3*spin + colour.
+ * O15: eta_k(x) = (g0 + i g1)/sqrt(2) with (g0, g1) the Box-Muller pair of generator block
+ * (site s, 64 + k, stream_id, purpose 4), so that <|eta_k|^2> = 1 and the weight is exp(-eta^dag eta). */
+int orc_spinor_gaussian(const int L[4], int subset, uint64_t seed, uint32_t stream_id, double *eta) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !eta || subset < 0 || subset > 2) return 1;
+    const double isq2 = 1.0 / sqrt(2.0);
+    for (long s = 0; s < lat.V; s++) {
+        if (!in_subset(&lat, s, subset)) continue;
+        for (int k = 0; k < 12; k++) {
+            double g[2];
+            orc_rng_block(seed, (uint32_t)s, 4u, (uint32_t)k, stream_id, 4u, NULL, NULL, g);
+            eta[((size_t)s * 12 + k) * 2 + 0] = g[0] * isq2;
+            eta[((size_t)s * 12 + k) * 2 + 1] = g[1] * isq2;
+        }
+    }
+    return 0;
+}
+
+/* O16: <a, b> = sum over the subset's sites and the nc complex components of conj(a) b; out = (Re, Im).
+ * Fields double[V][nc][2].  Serial, long double, lexicographic order. */
+int orc_inner_product(const int L[4], int subset, int nc, const double *a, const double *b, double out[2]) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !a || !b || !out || subset < 0 || subset > 2 || nc < 1) return 1;
+    long double re = 0, im = 0;
+    for (long s = 0; s < lat.V; s++) {
+        if (!in_subset(&lat, s, subset)) continue;
+        for (int k = 0; k < nc; k++) {
+            const double ar = a[((size_t)s * nc + k) * 2], ai = a[((size_t)s * nc + k) * 2 + 1];
+            const double br = b[((size_t)s * nc + k) * 2], bi = b[((size_t)s * nc + k) * 2 + 1];
+            re += (long double)ar * br + (long double)ai * bi;
+            im += (long double)ar * bi - (long double)ai * br;
+        }
+    }
+    out[0] = (double)re;
+    out[1] = (double)im;
+    return 0;
+}
+
+/* the same per timeslice ("sumMulti"): out[Lt][2] */
+int orc_inner_product_multi(const int L[4], int nc, const double *a, const double *b, double *out) {
+    lat_t lat;
+    if (lat_init(&lat, L) || !a || !b || !out || nc < 1) return 1;
+    int Lt = lat.L[3];
+    long Vs = lat.V / Lt;
+    for (int t = 0; t < Lt; t++) {
+        long double re = 0, im = 0;
+        for (long s = (long)t * Vs; s < (long)(t + 1) * Vs; s++)
+            for (int k = 0; k < nc; k++) {
+                const double ar = a[((size_t)s * nc + k) * 2], ai = a[((size_t)s * nc + k) * 2 + 1];
+                const double br = b[((size_t)s * nc + k) * 2], bi = b[((size_t)s * nc + k) * 2 + 1];
+                re += (long double)ar * br + (long double)ai * bi;
+                im += (long double)ar * bi - (long double)ai * br;
+            }
+        out[2 * t] = (double)re;
+        out[2 * t + 1] = (double)im;
+    }
+    return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -98,6 +98,13 @@ int orc_gauge_force_aniso(const int L[4], int subset, double beta_s, double beta
 int orc_nested_leapfrog(const int L[4], const double bs[2], const double bt[2], double tau, int n_outer,
                         int n_inner, double *U, double *P);
 
+/* O15 / O16 pseudofermion-side site operations (R21): spin-colour vector fields double[V][12][2].
+ * eta_k(x) = (g0 + i g1)/sqrt(2) from generator block (s, 64 + k, stream_id, purpose 4). */
+int orc_spinor_gaussian(const int L[4], int subset, uint64_t seed, uint32_t stream_id, double *eta);
+/* <a, b> = sum conj(a) b over the subset and nc complex components per site; out = (Re, Im) */
+int orc_inner_product(const int L[4], int subset, int nc, const double *a, const double *b, double out[2]);
+int orc_inner_product_multi(const int L[4], int nc, const double *a, const double *b, double *out /*[Lt][2]*/);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus
