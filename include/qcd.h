@@ -196,6 +196,26 @@ int qcd_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *ou
 int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2], const double beta_t[2],
                         double tau, int n_outer, int n_inner, void *U, void *P, void *stream);
 
+/* ---- pseudofermion-side site operations ("a pseudofermion refresh") ----
+ * Only the site-parallel pieces outside the Dirac operator (which, with the solver, is out of scope:
+ * PAPER.md:83): Gaussian fill of a spin-colour vector field and its norm / inner-product reductions
+ * (PAPER.md:26).  A spin-colour vector has 12 complex components per site, k = 3*spin + colour; device
+ * layout: complex pairs, component k of checkerboard site cb at pair index k*V + cb (24 reals per site;
+ * qcd_pack / qcd_unpack use this pair layout whenever ncomp is a multiple of 18 or of 24; canonical
+ * layout [s][k][re,im]).  [O15] eta_k(x) = (g0 + i g1)/sqrt(2), (g0,g1) the Box-Muller pair of generator
+ * block (lexicographic site, 64 + k, stream_id, purpose 4): <|eta_k|^2> = 1, weight exp(-eta^dag eta).
+ * Writes only the subset's sites.  The norm is qcd_sum(QCD_SUM_NORM2, ncomp = 24). */
+int qcd_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id,
+                        void *eta, void *stream);
+/* [O16] out[0], out[1] (device doubles) = Re, Im of <a,b> = sum over the subset's sites and the nc complex
+ * components per site of conj(a) b; a, b: pair-layout fields with nc components (12 for spin-colour
+ * vectors, 36 for the matrix fields).  fp64 accumulation, deterministic two-pass reduction like qcd_sum. */
+int qcd_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b,
+                      double *out, void *workspace, void *stream);
+/* the same per timeslice ("sumMulti"): out is device double[Lt][2] */
+int qcd_inner_product_multi(const qcd_lattice *lat, int prec, int nc, const void *a, const void *b, double *out,
+                            void *workspace, void *stream);
+
 /* ---- launch-parameter database of the auto-tuner (section 4) -------
  * The paper times every kernel as a function of the threads per block N_t and stores the best value in a
  * database.  Here the measuring lives in paper_1212_0785_b200/autotune.py (it calls the public kernels);

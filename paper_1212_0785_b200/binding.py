@@ -49,6 +49,9 @@ SIGNATURES = {
     "qcd_plaquette_st": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
     "qcd_nested_leapfrog": (_i, [_vp, _i, C.POINTER(C.c_double * 2), C.POINTER(C.c_double * 2), _d, _i, _i, _vp, _vp,
                                  _vp]),
+    "qcd_spinor_gaussian": (_i, [_vp, _i, _i, _u64, _u32, _vp, _vp]),
+    "qcd_inner_product": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_inner_product_multi": (_i, [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "qcd_tune_set": (_i, [_vp, _i, _i, _i, _i, C.POINTER(C.c_int * 4), _i]),
     "qcd_tune_get": (_i, [_vp, _i, _i, _i, C.POINTER(_i), C.POINTER(C.c_int * 4), C.POINTER(_i)]),
     "qcd_tune_clear": (_i, []),
@@ -140,6 +143,10 @@ class Lattice:
         """[36][V][2]: entry (mu*9+e, cb, re/im)"""
         return torch.empty((36, self.V, 2), dtype=dtype, device=device)
 
+    def new_spinor_field(self, dtype=torch.float64, device="cuda"):
+        """[12][V][2]: spin-colour component k = 3*spin + colour, site cb, re/im"""
+        return torch.empty((12, self.V, 2), dtype=dtype, device=device)
+
     def new_real_field(self, ncomp, dtype=torch.float64, device="cuda"):
         return torch.empty((ncomp, self.V), dtype=dtype, device=device)
 
@@ -225,6 +232,20 @@ def qcd_nested_leapfrog(lat, U, P, beta_s, beta_t, tau, n_outer, n_inner, stream
     bs, bt = (C.c_double * 2)(*beta_s), (C.c_double * 2)(*beta_t)
     _check(lib.qcd_nested_leapfrog(lat.handle, _prec(U), C.byref(bs), C.byref(bt), tau, n_outer, n_inner, _ptr(U),
                                    _ptr(P), _stream(stream)))
+
+
+def qcd_spinor_gaussian(lat, eta, seed, stream_id=0, subset=ALL, stream=None):
+    _check(lib.qcd_spinor_gaussian(lat.handle, _prec(eta), subset, seed, stream_id, _ptr(eta), _stream(stream)))
+
+
+def qcd_inner_product(lat, nc, a, b, out, workspace, subset=ALL, stream=None):
+    _check(lib.qcd_inner_product(lat.handle, _prec(a), subset, nc, _ptr(a), _ptr(b), _ptr(out), _ptr(workspace),
+                                 _stream(stream)))
+
+
+def qcd_inner_product_multi(lat, nc, a, b, out, workspace, stream=None):
+    _check(lib.qcd_inner_product_multi(lat.handle, _prec(a), nc, _ptr(a), _ptr(b), _ptr(out), _ptr(workspace),
+                                       _stream(stream)))
 
 
 def qcd_tune_set(lat, prec, subset, kernel, variant=0, tile=None, threads=0):

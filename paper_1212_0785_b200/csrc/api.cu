@@ -185,7 +185,9 @@ static int check_sum_args(int kind, int ncomp, const char *fn) {
     if (kind != QCD_SUM_SCALAR && kind != QCD_SUM_NORM2 && kind != QCD_SUM_RETR) return bad(QCD_EINVAL, "%s: unknown kind", fn);
     if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
     if (kind == QCD_SUM_SCALAR && ncomp > MAX_SUM_NCOMP) return bad(QCD_EINVAL, "%s: ncomp > 64 for SCALAR", fn);
-    if (kind != QCD_SUM_SCALAR && ncomp % 18) return bad(QCD_EINVAL, "%s: matrix kinds need ncomp %% 18 == 0", fn);
+    if (kind == QCD_SUM_RETR && ncomp % 18) return bad(QCD_EINVAL, "%s: RETR needs ncomp %% 18 == 0", fn);
+    if (kind == QCD_SUM_NORM2 && ncomp % 18 && ncomp % 24)
+        return bad(QCD_EINVAL, "%s: NORM2 needs a complex-pair field (ncomp %% 18 == 0 or ncomp %% 24 == 0)", fn);
     return QCD_OK;
 }
 
@@ -345,6 +347,40 @@ int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2]
             else QCD_TRY(kick(0.5 * e0, 0.5 * e1));
         }
     return QCD_OK;
+}
+
+int qcd_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
+                        void *stream) {
+    const char *fn = "qcd_spinor_gaussian";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_subset(subset, fn));
+    QCD_TRY(check_ptr(eta, fn));
+    return launch_spinor_gaussian(lat, prec, subset, seed, stream_id, eta, (cudaStream_t)stream);
+}
+
+static int check_inner(const qcd_lattice *lat, int prec, int nc, const void *a, const void *b, const double *out,
+                       const void *workspace, const char *fn) {
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(a, fn));
+    QCD_TRY(check_ptr(b, fn));
+    if (nc < 1) return bad(QCD_EINVAL, "%s: nc < 1", fn);
+    if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    return QCD_OK;
+}
+
+int qcd_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b, double *out,
+                      void *workspace, void *stream) {
+    const char *fn = "qcd_inner_product";
+    QCD_TRY(check_inner(lat, prec, nc, a, b, out, workspace, fn));
+    QCD_TRY(check_subset(subset, fn));
+    return launch_inner_product(lat, prec, subset, nc, a, b, false, out, (double *)workspace, (cudaStream_t)stream);
+}
+
+int qcd_inner_product_multi(const qcd_lattice *lat, int prec, int nc, const void *a, const void *b, double *out,
+                            void *workspace, void *stream) {
+    const char *fn = "qcd_inner_product_multi";
+    QCD_TRY(check_inner(lat, prec, nc, a, b, out, workspace, fn));
+    return launch_inner_product(lat, prec, QCD_ALL, nc, a, b, true, out, (double *)workspace, (cudaStream_t)stream);
 }
 
 int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int variant, const int tile[4],

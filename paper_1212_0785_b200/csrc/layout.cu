@@ -98,7 +98,7 @@ __global__ void map_kernel(const LatP lat, const int which, int32_t *__restrict_
 
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *src, void *dst, bool unpack,
                 cudaStream_t st) {
-    const bool matrix = ncomp % 18 == 0;
+    const bool matrix = ncomp % 18 == 0 || ncomp % 24 == 0;  // complex-pair layout: colour matrices, spin-colour vectors
     const size_t rb = prec == QCD_F64 ? 8 : 4;
     const size_t shm = (size_t)PK_SITES * (ncomp + 2) * rb;
     if (shm <= 48 * 1024) {  // transpose through shared memory; larger ncomp falls back to the direct kernel

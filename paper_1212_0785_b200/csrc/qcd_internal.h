@@ -95,6 +95,10 @@ int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp
                double *ws, cudaStream_t st);
 int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
                      const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st);
+int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
+                           cudaStream_t st);
+int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b,
+                         bool per_t, double *out, double *ws, cudaStream_t st);
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex, void *soa, bool unpack,
                 cudaStream_t st);
 int launch_get_map(const qcd_lattice *lat, int which, int32_t *out, cudaStream_t st);

@@ -63,6 +63,38 @@ __global__ void __launch_bounds__(128) perturb_kernel(const LatP lat, const uint
     }
 }
 
+// O15: spin-colour Gaussian fill, component k = blockIdx.y: eta_k(x) = (g0 + i g1)/sqrt(2) of generator block
+// (site, 64 + k, stream_id, purpose 4); pair layout, component k of site cb at pair index k*V + cb
+template <typename T>
+__global__ void __launch_bounds__(128) spinor_gauss_kernel(const LatP lat, const int begin, const int count,
+                                                           const uint64_t seed, const uint32_t stream_id,
+                                                           pair_t<T> *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const int cb = begin + i;
+    const int k = blockIdx.y;
+    const Site st = site_of_cb(lat, cb);
+    uint32_t w[4];
+    double u[2], g[2];
+    rng_block(seed, (uint32_t)st.s, (uint32_t)(64 + k), stream_id, 4u, w, u, g);
+    const double isq2 = 0.70710678118654752440;
+    pair_t<T> v;
+    v.x = (T)(g[0] * isq2);
+    v.y = (T)(g[1] * isq2);
+    out[(size_t)k * lat.V + cb] = v;
+}
+
+int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
+                           cudaStream_t st) {
+    int begin, count;
+    subset_range(lat->p, subset, begin, count);
+    const int threads = 128;
+    const dim3 grid((count + threads - 1) / threads, 12);
+    if (prec == QCD_F64) spinor_gauss_kernel<double><<<grid, threads, 0, st>>>(lat->p, begin, count, seed, stream_id, (double2 *)eta);
+    else spinor_gauss_kernel<float><<<grid, threads, 0, st>>>(lat->p, begin, count, seed, stream_id, (float2 *)eta);
+    return check_launch("spinor_gaussian");
+}
+
 __global__ void rng_blocks_kernel(const uint64_t seed, const uint32_t stream_id, const uint32_t purpose, const int n,
                                   const uint32_t *__restrict__ site, const uint32_t *__restrict__ mu_j,
                                   uint32_t *__restrict__ words, double *__restrict__ uniforms,

@@ -61,10 +61,25 @@ __device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T
     return (double)acc;
 }
 
+// QCD_SUM_INNER (kind 3, internal): comp 0 / 1 = Re / Im of sum_k conj(a_k) b_k over the ncomp/2 complex
+// components of two pair-layout fields (O16)
+constexpr int SUM_INNER = 3;
+
 template <typename T>
-__device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int V, const T *__restrict__ f, int cb) {
+__device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int V, const T *__restrict__ f, int cb,
+                                             const T *__restrict__ f2 = nullptr) {
     if (kind == QCD_SUM_SCALAR) return (double)__ldg(f + (size_t)comp * V + cb);
     double acc = 0.0;
+    if (kind == SUM_INNER) {
+        const pair_t<T> *a = (const pair_t<T> *)f, *b = (const pair_t<T> *)f2;
+        for (int k = 0; k < ncomp / 2; k++) {
+            const pair_t<T> x = __ldg(a + (size_t)k * V + cb), y = __ldg(b + (size_t)k * V + cb);
+            if (comp == 0) acc = fma((double)x.x, (double)y.x, fma((double)x.y, (double)y.y, acc));
+            else  // both products rounded before the difference (no FMA contraction): Im <a,a> is exactly 0
+                acc += __dsub_rn(__dmul_rn((double)x.x, (double)y.y), __dmul_rn((double)x.y, (double)y.x));
+        }
+        return acc;
+    }
     if (kind == QCD_SUM_NORM2) {
         const pair_t<T> *p = (const pair_t<T> *)f;
         for (int k = 0; k < ncomp / 2; k++) {
@@ -90,7 +105,8 @@ __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int 
 // partial[(comp*nseg + seg)*cps + chunk], seg = 2*t + parity
 template <typename T>
 __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, const int kind, const int ncomp,
-                                                            const void *__restrict__ field, double *__restrict__ partial) {
+                                                            const void *__restrict__ field, double *__restrict__ partial,
+                                                            const void *__restrict__ field2 = nullptr) {
     const int cps = gridDim.x, nseg = gridDim.y;
     const int seg = blockIdx.y, comp = blockIdx.z;
     const int Vsh = lat.Vh / lat.L[3];
@@ -102,7 +118,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, cons
         if (i < Vsh) {
             const int cb = seg_begin + i;
             acc += kind < 0 ? site_plaquette<T>(lat, (const pair_t<T> *)field, cb, kind == -1 ? 0 : 1 + comp)
-                            : site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb);
+                            : site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb, (const T *)field2);
         }
     }
     const double r = block_sum(acc);
@@ -219,6 +235,28 @@ int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp
                double *ws, cudaStream_t st) {
     return prec == QCD_F64 ? sum_t<double>(lat, subset, kind, ncomp, field, out, ws, st)
                            : sum_t<float>(lat, subset, kind, ncomp, field, out, ws, st);
+}
+
+// O16: out[0], out[1] = Re, Im of <a, b> over the subset; per_t = true: out[t*2 + {0,1}] per timeslice
+template <typename T>
+static int inner_t(const qcd_lattice *lat, int subset, int nc, const void *a, const void *b, bool per_t, double *out,
+                   double *ws, cudaStream_t st) {
+    const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
+    reduce_pass1<T><<<dim3(cps, nseg, 2), RED_THREADS, 0, st>>>(lat->p, SUM_INNER, 2 * nc, a, ws, b);
+    if (per_t) {
+        const int Lt = lat->p.L[3];
+        reduce_pass2<<<dim3(Lt, 2), RED_THREADS, 0, st>>>(ws, Lt, 2 * cps, 1.0, out, 2);
+    } else {
+        const int par = subset == QCD_ALL ? 2 : subset == QCD_EVEN ? 0 : 1;
+        reduce_pass2_global<<<2, RED_THREADS, 0, st>>>(ws, nseg, cps, par, 1.0, out);
+    }
+    return check_launch("inner_product");
+}
+
+int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b,
+                         bool per_t, double *out, double *ws, cudaStream_t st) {
+    return prec == QCD_F64 ? inner_t<double>(lat, subset, nc, a, b, per_t, out, ws, st)
+                           : inner_t<float>(lat, subset, nc, a, b, per_t, out, ws, st);
 }
 
 template <typename T>
