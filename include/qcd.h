@@ -157,6 +157,20 @@ int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const v
 int qcd_md_step(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, void *U,
                 void *P, void *stream);
 
+/* qcd_force_mom_update on the whole lattice with the two sums of the Hamiltonian as by-products (reductions
+ * of PAPER.md:26 fused into the site loop): out[0] = plaquette average of U (as qcd_plaquette's
+ * out_avg: sum_{x,mu} Re tr W_mu(x) = 4 sum_{x,mu<nu} Re tr P_mu_nu(x)), out[1] = K = sum |P_ij|^2 of the
+ * UPDATED momenta (as qcd_sum NORM2).  Saves the two extra passes (1152 B/site) per observed step.  Device
+ * doubles; workspace as qcd_workspace_bytes.  Deterministic run to run at a fixed block shape (one partial
+ * per block, fixed order); not per timeslice.  QCD_EWORKSPACE if the lattice's workspace cannot hold
+ * two doubles per block. */
+int qcd_force_mom_update_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P,
+                              double *out, void *workspace, void *stream);
+/* qcd_leapfrog whose last momentum update is qcd_force_mom_update_sums: out[0] = plaquette average and
+ * out[1] = K at the END of the trajectory, i.e. H_end = out[1] + beta*6V*(1 - out[0]) at no extra pass. */
+int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
+                        double *out, void *workspace, void *stream);
+
 /* The same MD step in ONE pass over the lattice (SURVEY.md 8(a) "single pass, ping-pong U"; loop fusion
  * in the sense of PAPER.md:32): P <- P + eps_p*F(U_in); U_out <- reunit(exp(i eps_u P) U_in), one kernel.
  * U_in is only read; U_out is a second gauge field of the same size that must not overlap U_in or P

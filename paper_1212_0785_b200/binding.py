@@ -42,6 +42,8 @@ SIGNATURES = {
     "qcd_sum_multi": (_i, [_vp, _i, _i, _i, _vp, _vp, _i, _vp, _vp, _vp]),
     "qcd_md_step": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp]),
     "qcd_leapfrog": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp]),
+    "qcd_force_mom_update_sums": (_i, [_vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_leapfrog_energy": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp, _vp]),
     "qcd_md_step_single_pass": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "qcd_leapfrog_single_pass": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
     "qcd_gauge_force_aniso": (_i, [_vp, _i, _i, _d, _d, _vp, _vp, _vp]),
@@ -201,6 +203,16 @@ def qcd_md_step(lat, U, P, beta, eps_p, eps_u, stream=None):
 
 def qcd_leapfrog(lat, U, P, beta, eps, nsteps, stream=None):
     _check(lib.qcd_leapfrog(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _stream(stream)))
+
+
+def qcd_force_mom_update_sums(lat, U, P, beta, eps, out, workspace, stream=None):
+    _check(lib.qcd_force_mom_update_sums(lat.handle, _prec(U), beta, eps, _ptr(U), _ptr(P), _ptr(out), _ptr(workspace),
+                                         _stream(stream)))
+
+
+def qcd_leapfrog_energy(lat, U, P, beta, eps, nsteps, out, workspace, stream=None):
+    _check(lib.qcd_leapfrog_energy(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _ptr(out), _ptr(workspace),
+                                   _stream(stream)))
 
 
 def qcd_md_step_single_pass(lat, U_in, P, U_out, beta, eps_p, eps_u, stream=None):

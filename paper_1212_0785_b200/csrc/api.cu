@@ -88,7 +88,8 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
     lat->red_nseg = 2 * dims[3];
     const size_t a = (size_t)MAX_SUM_NCOMP * lat->red_nseg * lat->red_chunks_per_seg;
     const size_t b = (size_t)MAX_NSUB * RED_GENERIC_CHUNKS;
-    lat->workspace_doubles = (a > b ? a : b) + 64;
+    const size_t c = 2 * ((size_t)V / 32 + 1);  // per-block partial pairs of the kernels that reduce as a by-product
+    lat->workspace_doubles = (a > b ? (a > c ? a : c) : (b > c ? b : c)) + 64;
     *out = lat;
     return QCD_OK;
 }
@@ -243,6 +244,35 @@ int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int 
         QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, k == nsteps - 1 ? 0.5 * eps : eps, U, P, true, st));
     }
     return QCD_OK;
+}
+
+int qcd_force_mom_update_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P,
+                              double *out, void *workspace, void *stream) {
+    const char *fn = "qcd_force_mom_update_sums";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    return launch_force_sums(lat, prec, beta, eps, U, P, out, (double *)workspace, (cudaStream_t)stream);
+}
+
+int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
+                        double *out, void *workspace, void *stream) {
+    const char *fn = "qcd_leapfrog_energy";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
+    if (nsteps < 1) return bad(QCD_EINVAL, "%s: nsteps < 1", fn);
+    if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    cudaStream_t st = (cudaStream_t)stream;
+    QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, U, P, true, st));
+    for (int k = 0; k < nsteps; k++) {
+        QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
+        if (k < nsteps - 1) QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps, U, P, true, st));
+    }
+    return launch_force_sums(lat, prec, beta, 0.5 * eps, U, P, out, (double *)workspace, st);
 }
 
 int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,

@@ -11,6 +11,12 @@
 #include "site.cuh"
 #include "su3.cuh"
 
+#define QCD_TRY_RC(expr)               \
+    do {                               \
+        const int rc_ = (expr);        \
+        if (rc_ != QCD_OK) return rc_; \
+    } while (0)
+
 namespace qcd {
 
 // thread -> site of the block's tile
@@ -58,11 +64,16 @@ __device__ __forceinline__ void ldU(M3<T> &m, const pair_t<T> *__restrict__ f, i
 // wt if mu or nu is the time direction, else ws (c is then 1/12); planes of weight zero are skipped, which
 // is what the levels of the multi-timescale integrator (space-space planes only / space-time planes only) use.
 template <typename T, bool FUSED, bool EARLYP, bool LINK, int NT = 256, int MINB = 1, bool REC = false,
-          bool ANISO = false>
+          bool ANISO = false, bool SUMS = false>
 __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */,
                                                     const T eps, const pair_t<T> *__restrict__ U,
                                                     pair_t<T> *__restrict__ out, const T eps_u,
-                                                    pair_t<T> *__restrict__ Uout, const T ws, const T wt) {
+                                                    pair_t<T> *__restrict__ Uout, const T ws, const T wt,
+                                                    double *__restrict__ partial = nullptr) {
+    // SUMS (needs FUSED): the two sums the Hamiltonian needs are by-products (PAPER.md:26 reductions, fused
+    // as in PAPER.md:32): sum Re tr W_mu(x) = 4 sum_{mu<nu} Re tr P_mu_nu (every plaquette closes four staple
+    // loops) and K = sum |P_ij|^2 of the updated momenta.  One fp64 partial pair per block, fixed order.
+    double sumW = 0.0, sumK = 0.0;
     const Site st = tile_site(lat, tile, threadIdx.x);
     const int V = lat.V;
     const int par = st.par;
@@ -124,6 +135,14 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
                 P.im[e] = fma_(eps, F.im[e], P.im[e]);
             }
             store_link_cs(P, out, V, mu, cb);
+            if (SUMS) {
+                sumW += (double)W.re[0] + (double)W.re[4] + (double)W.re[8];
+#pragma unroll
+                for (int e = 0; e < 9; e++) {
+                    sumK = fma((double)P.re[e], (double)P.re[e], sumK);
+                    sumK = fma((double)P.im[e], (double)P.im[e], sumK);
+                }
+            }
             if (LINK) {
 #pragma unroll
                 for (int e = 0; e < 9; e++) {
@@ -138,6 +157,28 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
             }
         } else {
             store_link_cs(F, out, V, mu, cb);
+        }
+    }
+    if (SUMS) {
+        __shared__ double part[2][NT / 32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sumW += __shfl_down_sync(0xffffffffu, sumW, o);
+            sumK += __shfl_down_sync(0xffffffffu, sumK, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            part[0][threadIdx.x >> 5] = sumW;
+            part[1][threadIdx.x >> 5] = sumK;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double a = 0.0, b = 0.0;
+            for (int w = 0; w < (int)(blockDim.x + 31) / 32; w++) {
+                a += part[0][w];
+                b += part[1][w];
+            }
+            partial[blockIdx.x] = a;
+            partial[gridDim.x + blockIdx.x] = b;
         }
     }
 }
@@ -600,6 +641,30 @@ int launch_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, doubl
                              const void *U, void *out, bool fused_mom, cudaStream_t st) {
     return prec == QCD_F64 ? launch_force_aniso_t<double>(lat, subset, ws, wt, eps, U, out, fused_mom, st)
                            : launch_force_aniso_t<float>(lat, subset, ws, wt, eps, U, out, fused_mom, st);
+}
+
+// Force + momentum update with the plaquette and kinetic-energy sums as by-products (subset ALL).
+// out[0] = plaquette average of U, out[1] = K of the updated P.  ws: 2 x blocks doubles.
+template <typename T>
+static int launch_force_sums_t(const qcd_lattice *lat, double beta, double eps, const void *U, void *P, double *out,
+                               double *ws, cudaStream_t st) {
+    const TileP tp = choose_tile(lat->p, QCD_ALL, 128);
+    const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
+    if ((size_t)2 * blocks > lat->workspace_doubles) {
+        set_error("force_mom_update_sums: workspace too small");
+        return QCD_EWORKSPACE;
+    }
+    force_kernel<T, true, false, false, 128, 3, false, false, true><<<blocks, tp.tsp * tp.npar, 0, st>>>(
+        lat->p, tp, (T)(beta / 12.0), (T)eps, (const pair_t<T> *)U, (pair_t<T> *)P, T(0), nullptr, T(0), T(0), ws);
+    QCD_TRY_RC(check_launch("force_mom_update_sums"));
+    QCD_TRY_RC(launch_sum_partials(ws, blocks, 1.0 / (72.0 * (double)lat->p.V), out, st));
+    return launch_sum_partials(ws + blocks, blocks, 1.0, out + 1, st);
+}
+
+int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P, double *out,
+                      double *ws, cudaStream_t st) {
+    return prec == QCD_F64 ? launch_force_sums_t<double>(lat, beta, eps, U, P, out, ws, st)
+                           : launch_force_sums_t<float>(lat, beta, eps, U, P, out, ws, st);
 }
 
 // Single-pass MD step: P += eps_p F(U); Uout = reunit(exp(i eps_u P) U).  Subset ALL only (every link moves).

@@ -95,6 +95,10 @@ int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp
                double *ws, cudaStream_t st);
 int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
                      const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st);
+// force + momentum update with plaquette and kinetic-energy sums as by-products (force.cu); ws: 2*blocks doubles
+int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P, double *out,
+                      double *ws, cudaStream_t st);
+int launch_sum_partials(const double *partial, int count, double scale, double *out, cudaStream_t st);
 int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
                            cudaStream_t st);
 int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b,

@@ -625,3 +625,48 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
     K = torch.zeros(1, dtype=torch.float64, device="cuda")
     qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, dP, K, ws)
     assert abs(K.item() / (16 * lat.V) - 1) < 0.01
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (6, 4, 2, 8), (12, 6, 10, 4), (16, 16, 16, 32)])
+def test_force_mom_update_with_fused_sums(qcd, orc_omp, prec, dims):
+    """plaquette and kinetic energy as by-products of the force kernel (sum rule: sum Re tr W = 4 sum Re tr P)"""
+    import torch
+    lat = qcd.Lattice(dims)
+    beta, eps = 5.9, 0.04
+    U = round_to(prec, orc_omp.hot_start(dims, 91, 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, 92))
+    dU, dP = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec)
+    ws = lat.new_workspace()
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    qcd.qcd_force_mom_update_sums(lat, dU, dP, beta, eps, out, ws)
+    P1 = orc_omp.mom_update(dims, eps, orc_omp.gauge_force(dims, beta, U), P)
+    assert rel(host(qcd, lat, dP), P1) < TOL[prec]
+    plaq, K = out.cpu().numpy()
+    rplaq = orc_omp.plaquette(dims, U)[0]
+    rK = orc_omp.sum(dims, O.SUM_NORM2, P1.view(np.float64).reshape(lat.V, 72))
+    assert abs(plaq - rplaq) < TOL[prec] * abs(rplaq) and abs(K - rK) < TOL[prec] * rK
+    # deterministic, and the same numbers as the stand-alone reductions up to rounding order
+    dP2 = dev(qcd, lat, P, prec)
+    out2 = torch.zeros(2, dtype=torch.float64, device="cuda")
+    qcd.qcd_force_mom_update_sums(lat, dU, dP2, beta, eps, out2, ws)
+    assert torch.equal(out, out2) and torch.equal(dP, dP2)
+
+
+def test_leapfrog_energy_gives_the_final_hamiltonian(qcd, orc_omp):
+    import torch
+    c = inputs.CONFIGS[2]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    lat = qcd.Lattice(dims)
+    U = orc_omp.hot_start(dims, inputs.config_seed(2), c["sigma"])
+    P = orc_omp.mom_refresh(dims, inputs.config_seed(2))
+    dU, dP = dev(qcd, lat, U, "f64"), dev(qcd, lat, P, "f64")
+    ws = lat.new_workspace()
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    qcd.qcd_leapfrog_energy(lat, dU, dP, beta, eps, 4, out, ws)
+    U1, P1 = orc_omp.leapfrog(dims, beta, eps, 4, U, P)
+    assert rel(host(qcd, lat, dU), U1) < 1e-12 and rel(host(qcd, lat, dP), P1) < 1e-12
+    rK, rS = orc_omp.hamiltonian(dims, beta, U1, P1)
+    plaq, K = out.cpu().numpy()
+    H = K + beta * 6 * lat.V * (1 - plaq)
+    assert abs(H - (rK + rS)) < 1e-12 * abs(rK + rS)
