@@ -279,7 +279,10 @@ def run_ours(args, cfg):
                                 {"force_mom_update": force_ms, "link_update_reunit": link_ms}},
         "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": force_bytes},
+                     "algorithmic_bytes_per_launch": force_bytes,
+                     # the same kernel against the plain-ALU roofline it also sits near: FMA per site x V
+                     # / time over the nominal 148 SMs x 64 (fp64) or 128 (fp32) lanes x 1.965 GHz
+                     "fma_frac": (5616 + 222 + (4 * 550 if single else 0)) * V / (force_ms * 1e-3) / FMA_PEAK[args.dtype]},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * fb, "d2h_bytes_per_step": 2 * fb,
                 "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout)"},
         "gpu_launches": K if single else 2 * K,
@@ -298,6 +301,97 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+# per-kernel table: reals per site read + written, FMA per site (products x 108 + small)
+KERNEL_TABLE = [
+    # name, reals/site, FMA/site, subsets
+    ("gauge_force", 144, 5616 + 150, True),
+    ("mom_update", 216, 72, True),
+    ("force_mom_update", 216, 5616 + 222, True),
+    ("link_update", 216, 4 * 410, True),
+    ("reunit", 144, 4 * 150, True),
+    ("link_update_reunit", 216, 4 * 550, True),
+    ("mom_refresh", 72, 0, True),
+    ("plaquette", 72, 12 * 108 + 6 * 18, False),
+    ("sum_norm2", 72, 72, True),
+    ("sum_multi_norm2_per_t", 72, 72, False),
+    ("md_step_single_pass", 288, 5616 + 222 + 4 * 550, False),
+    ("force_mom_update_sums", 216, 5616 + 330, False),
+]
+FMA_PEAK = {"f64": 148 * 64 * 1.965e9, "f32": 148 * 128 * 1.965e9}  # nominal lanes x clock
+
+
+def run_per_kernel(args, cfg):
+    """each kernel alone on ALL / EVEN / ODD with an L2 flush between timed launches (config 3's U + P is about the
+    size of L2); one JSON line with a list of rows"""
+    import torch
+
+    from paper_1212_0785_b200 import binding as qcd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dtype = torch.float64 if args.dtype == "f64" else torch.float32
+    rb = 8 if args.dtype == "f64" else 4
+    dims, beta, eps = cfg["dims"], cfg["beta"], cfg["eps"]
+    lat = qcd.Lattice(dims)
+    V = lat.V
+    U, P, F, W = (lat.new_matrix_field(dtype) for _ in range(4))
+    ws = lat.new_workspace()
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")  # 4 x L2
+    peak, peak_src = peaks()
+    stream = torch.cuda.current_stream()
+
+    def reset():
+        qcd.qcd_hot_start(lat, U, SEED_BASE + args.config, cfg["sigma"])
+        qcd.qcd_perturb(lat, U, SEED_BASE + args.config, 1e-3)  # config 3: reunit input off SU(3) by sigma = 1e-3
+        qcd.qcd_mom_refresh(lat, P, SEED_BASE + args.config)
+        qcd.qcd_mom_refresh(lat, F, SEED_BASE + args.config, stream_id=1)
+
+    calls = {
+        "gauge_force": lambda sub: qcd.qcd_gauge_force(lat, U, F, beta, subset=sub),
+        "mom_update": lambda sub: qcd.qcd_mom_update(lat, F, P, eps, subset=sub),
+        "force_mom_update": lambda sub: qcd.qcd_force_mom_update(lat, U, P, beta, eps, subset=sub),
+        "link_update": lambda sub: qcd.qcd_link_update(lat, P, U, eps, reunit=False, subset=sub),
+        "reunit": lambda sub: qcd.qcd_reunit(lat, U, subset=sub),
+        "link_update_reunit": lambda sub: qcd.qcd_link_update(lat, P, U, eps, reunit=True, subset=sub),
+        "mom_refresh": lambda sub: qcd.qcd_mom_refresh(lat, P, SEED_BASE, subset=sub),
+        "plaquette": lambda sub: qcd.qcd_plaquette(lat, U, out[0:1], per_t, ws),
+        "sum_norm2": lambda sub: qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, P, out[1:2], ws, subset=sub),
+        "sum_multi_norm2_per_t": lambda sub: qcd.qcd_sum_multi(lat, qcd.SUM_NORM2, 72, P, None, dims[3], per_t, ws),
+        "md_step_single_pass": lambda sub: qcd.qcd_md_step_single_pass(lat, U, P, W, beta, eps, eps),
+        "force_mom_update_sums": lambda sub: qcd.qcd_force_mom_update_sums(lat, U, P, beta, eps, out, ws),
+    }
+    rows = []
+    reps = max(5, min(args.steps, 20))
+    for name, reals, fma, has_subsets in KERNEL_TABLE:
+        for sub, sname in ((qcd.ALL, "all"), (qcd.EVEN, "even"), (qcd.ODD, "odd")):
+            if sub != qcd.ALL and not has_subsets:
+                continue
+            reset()
+            fn = calls[name]
+            for _ in range(3):
+                fn(sub)
+            ts = []
+            for _ in range(reps):
+                flush.fill_(1)  # evict the fields from L2
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fn(sub)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            ts.sort()
+            ms = ts[len(ts) // 2]
+            sites = V if sub == qcd.ALL else V // 2
+            gbs = reals * rb * sites / (ms * 1e-3) / 1e9
+            rows.append({"kernel": name, "subset": sname, "ms": ms, "bytes_per_site": reals * rb, "gbs": gbs,
+                         "frac_hbm": gbs / peak, "site_updates_per_s": sites / (ms * 1e-3),
+                         "frac_fma": fma * sites / (ms * 1e-3) / FMA_PEAK[args.dtype]})
+    print(json.dumps({"per_kernel": rows, "config": {"workload": f"{cfg['name']} {args.dtype}, each kernel alone, "
+                      "L2 flushed (512 MB write) before every timed launch", "reps": reps},
+                      "peak_gbs": peak, "peak_source": peak_src, "fma_peak": FMA_PEAK[args.dtype]}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -311,11 +405,16 @@ def main():
                          "one as measured); single_pass: qcd_md_step_single_pass ping-ponging two gauge fields")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-kernel", action="store_true",
+                    help="instead of the MD-step line: every kernel alone on ALL/EVEN/ODD with an L2 flush between "
+                         "launches (SURVEY.md 8(d), config 3 row); prints one JSON object with the table")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.per_kernel:
+        run_per_kernel(args, cfg)
     else:
         run_ours(args, cfg)
 

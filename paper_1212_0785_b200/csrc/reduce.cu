@@ -106,9 +106,12 @@ __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int 
 template <typename T>
 __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, const int kind, const int ncomp,
                                                             const void *__restrict__ field, double *__restrict__ partial,
-                                                            const void *__restrict__ field2 = nullptr) {
-    const int cps = gridDim.x, nseg = gridDim.y;
-    const int seg = blockIdx.y, comp = blockIdx.z;
+                                                            const void *__restrict__ field2 = nullptr,
+                                                            const int par_only = -1) {
+    // par_only = 0 / 1: a parity subset — only that parity's segments are visited (grid.y = Lt), the partial
+    // array keeps its full (2 Lt segment) indexing so the second pass is the same
+    const int cps = gridDim.x, nseg = par_only < 0 ? gridDim.y : 2 * gridDim.y;
+    const int seg = par_only < 0 ? blockIdx.y : 2 * blockIdx.y + par_only, comp = blockIdx.z;
     const int Vsh = lat.Vh / lat.L[3];
     const int seg_begin = (seg & 1) * lat.Vh + (seg >> 1) * Vsh;
     double acc = 0.0;
@@ -232,8 +235,9 @@ static int sum_t(const qcd_lattice *lat, int subset, int kind, int ncomp, const 
                  cudaStream_t st) {
     const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
     const int nout = kind == QCD_SUM_SCALAR ? ncomp : 1;
-    reduce_pass1<T><<<dim3(cps, nseg, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field, ws);
     const int par = subset == QCD_ALL ? 2 : subset == QCD_EVEN ? 0 : 1;
+    if (par == 2) reduce_pass1<T><<<dim3(cps, nseg, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field, ws);
+    else reduce_pass1<T><<<dim3(cps, nseg / 2, nout), RED_THREADS, 0, st>>>(lat->p, kind, ncomp, field, ws, nullptr, par);
     reduce_pass2_global<<<nout, RED_THREADS, 0, st>>>(ws, nseg, cps, par, 1.0, out);
     return check_launch("sum");
 }
@@ -249,12 +253,13 @@ template <typename T>
 static int inner_t(const qcd_lattice *lat, int subset, int nc, const void *a, const void *b, bool per_t, double *out,
                    double *ws, cudaStream_t st) {
     const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
-    reduce_pass1<T><<<dim3(cps, nseg, 2), RED_THREADS, 0, st>>>(lat->p, SUM_INNER, 2 * nc, a, ws, b);
+    const int par = subset == QCD_ALL ? 2 : subset == QCD_EVEN ? 0 : 1;
+    if (par == 2 || per_t) reduce_pass1<T><<<dim3(cps, nseg, 2), RED_THREADS, 0, st>>>(lat->p, SUM_INNER, 2 * nc, a, ws, b);
+    else reduce_pass1<T><<<dim3(cps, nseg / 2, 2), RED_THREADS, 0, st>>>(lat->p, SUM_INNER, 2 * nc, a, ws, b, par);
     if (per_t) {
         const int Lt = lat->p.L[3];
         reduce_pass2<<<dim3(Lt, 2), RED_THREADS, 0, st>>>(ws, Lt, 2 * cps, 1.0, out, 2);
     } else {
-        const int par = subset == QCD_ALL ? 2 : subset == QCD_EVEN ? 0 : 1;
         reduce_pass2_global<<<2, RED_THREADS, 0, st>>>(ws, nseg, cps, par, 1.0, out);
     }
     return check_launch("inner_product");
