@@ -670,3 +670,28 @@ def test_leapfrog_energy_gives_the_final_hamiltonian(qcd, orc_omp):
     plaq, K = out.cpu().numpy()
     H = K + beta * 6 * lat.V * (1 - plaq)
     assert abs(H - (rK + rS)) < 1e-12 * abs(rK + rS)
+
+
+@pytest.mark.parametrize("n", [1, 2])
+def test_config_observables_against_stored_oracle_values(qcd, n):
+    """BASELINE configs 1 and 2: plaquette, kinetic energy and dH of the GPU trajectory (start generated on the
+    device, qcd_leapfrog_energy) against tests/golden/config_values.json, written by the oracle alone"""
+    import json
+    import os
+    import torch
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "config_values.json")))[str(n)]
+    dims, beta = tuple(g["dims"]), g["beta"]
+    seed = int(g["seed"], 16)
+    lat = qcd.Lattice(dims)
+    ws = lat.new_workspace()
+    dU, dP = lat.new_matrix_field(), lat.new_matrix_field()
+    qcd.qcd_hot_start(lat, dU, seed, g["sigma"])
+    qcd.qcd_mom_refresh(lat, dP, seed)
+    K0, S0, plaq0 = gpu_H(qcd, lat, dU, dP, beta, ws)
+    assert abs(plaq0 - g["plaq0"]) < 1e-12 and abs(K0 - g["K0"]) < 1e-12 * g["K0"] and abs(S0 - g["S0"]) < 1e-12 * g["S0"]
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    qcd.qcd_leapfrog_energy(lat, dU, dP, beta, g["eps"], g["nsteps"], out, ws)
+    plaq1, K1 = out.cpu().numpy()
+    S1 = beta * 6 * lat.V * (1 - plaq1)
+    assert abs(plaq1 - g["plaq1"]) < 1e-12 and abs(K1 - g["K1"]) < 1e-12 * g["K1"]
+    assert abs(((K1 + S1) - (K0 + S0)) - g["dH"]) <= 1e-12 * abs(g["K0"] + g["S0"])  # R15: dH against |H|

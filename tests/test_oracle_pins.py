@@ -495,3 +495,21 @@ def test_force_at_listed_sites_is_the_full_force(orc):
     F = orc.gauge_force(dims, 5.5, U)
     sites = np.array([0, 5, 127, 17, 5], dtype=np.int32)
     assert np.array_equal(orc.gauge_force_sites(dims, 5.5, U, sites), F[sites])
+
+
+def test_oracle_reproduces_stored_config_values(orc):
+    """tests/golden/config_values.json (written by tests/golden/make_config_values.py from the oracle alone):
+    the oracle still gives the same config-1 observables; hot-start plaquette near its expectation chi(sigma)^4"""
+    import json
+    g = json.load(open(os.path.join(GOLDEN, "config_values.json")))["1"]
+    dims, beta = tuple(g["dims"]), g["beta"]
+    seed = int(g["seed"], 16)
+    U0, P0 = orc.hot_start(dims, seed, g["sigma"]), orc.mom_refresh(dims, seed)
+    K0, S0 = orc.hamiltonian(dims, beta, U0, P0)
+    U1, P1 = orc.leapfrog(dims, beta, g["eps"], g["nsteps"], U0, P0)
+    K1, S1 = orc.hamiltonian(dims, beta, U1, P1)
+    assert np.isclose(orc.plaquette(dims, U0)[0], g["plaq0"], rtol=1e-13) and np.isclose(K0, g["K0"], rtol=1e-13)
+    assert np.isclose(orc.plaquette(dims, U1)[0], g["plaq1"], rtol=1e-13) and np.isclose(K1, g["K1"], rtol=1e-13)
+    assert abs(((K1 + S1) - (K0 + S0)) - g["dH"]) < 1e-9 * abs(K0 + S0)
+    assert abs(g["K0"] / (16 * np.prod(dims)) - 1) < 4 / np.sqrt(16 * np.prod(dims))  # <K> = 16 V
+    assert abs(g["plaq0"] - 0.503) < 0.03  # chi(0.5)^4 (SURVEY.md 8(c) pin table), 4^4 statistics
