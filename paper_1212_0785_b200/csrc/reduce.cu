@@ -21,8 +21,7 @@ __device__ __forceinline__ double block_sum(double v) {
     __syncthreads();
     double r = 0.0;
     if (threadIdx.x == 0) {
-#pragma unroll
-        for (int k = 0; k < RED_THREADS / 32; k++) r += warp_part[k];
+        for (int k = 0; k < (int)blockDim.x / 32; k++) r += warp_part[k];
     }
     __syncthreads();
     return r;
@@ -100,8 +99,7 @@ __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int 
 
 // ---- pass 1 --------------------------------------------------------------------------------
 
-// grid (chunks_per_seg, nseg, ncomp_out); kind = -1: plaquette; kind = -2: comp 0 = space-space planes,
-// comp 1 = space-time planes.
+// grid (chunks_per_seg, nseg, ncomp_out).
 // partial[(comp*nseg + seg)*cps + chunk], seg = 2*t + parity
 template <typename T>
 __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, const int kind, const int ncomp,
@@ -120,9 +118,30 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, cons
         const int i = blockIdx.x * RED_CHUNK + k * RED_THREADS + threadIdx.x;
         if (i < Vsh) {
             const int cb = seg_begin + i;
-            acc += kind < 0 ? site_plaquette<T>(lat, (const pair_t<T> *)field, cb, kind == -1 ? 0 : 1 + comp)
-                            : site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb, (const T *)field2);
+            acc += site_value<T>(kind, ncomp, comp, lat.V, (const T *)field, cb, (const T *)field2);
         }
+    }
+    const double r = block_sum(acc);
+    if (threadIdx.x == 0) partial[((size_t)comp * nseg + seg) * cps + blockIdx.x] = r;
+}
+
+// plaquette pass 1, same chunk geometry and partial layout as reduce_pass1 (grid (cps, nseg, ncomp_out)) but in
+// PLAQ_THREADS-thread blocks, several resident per SM: the stencil kernel wants warps, not wide blocks
+// (profiles/r01c_per_kernel.md).  which0: 0 = all planes; 1 = comp 0 space-space, comp 1 space-time.
+constexpr int PLAQ_THREADS = 128;
+template <typename T>
+__global__ void __launch_bounds__(PLAQ_THREADS, 3) plaquette_pass1(const LatP lat, const int which0,
+                                                                   const pair_t<T> *__restrict__ U,
+                                                                   double *__restrict__ partial) {
+    const int cps = gridDim.x, nseg = gridDim.y;
+    const int seg = blockIdx.y, comp = blockIdx.z;
+    const int Vsh = lat.Vh / lat.L[3];
+    const int seg_begin = (seg & 1) * lat.Vh + (seg >> 1) * Vsh;
+    double acc = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < RED_CHUNK / PLAQ_THREADS; k++) {
+        const int i = blockIdx.x * RED_CHUNK + k * PLAQ_THREADS + threadIdx.x;
+        if (i < Vsh) acc += site_plaquette<T>(lat, U, seg_begin + i, which0 ? 1 + comp : 0);
     }
     const double r = block_sum(acc);
     if (threadIdx.x == 0) partial[((size_t)comp * nseg + seg) * cps + blockIdx.x] = r;
@@ -188,7 +207,7 @@ static int plaquette_t(const qcd_lattice *lat, const void *U, double *out_avg, d
                        cudaStream_t st) {
     const LatP &p = lat->p;
     const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
-    reduce_pass1<T><<<dim3(cps, nseg, 1), RED_THREADS, 0, st>>>(p, -1, 72, U, ws);
+    plaquette_pass1<T><<<dim3(cps, nseg, 1), PLAQ_THREADS, 0, st>>>(p, 0, (const pair_t<T> *)U, ws);
     const int Lt = p.L[3];
     const double Vs = (double)(p.V / Lt);
     if (out_per_t)  // segments 2t, 2t+1 are adjacent: one group of 2*cps partials per timeslice
@@ -215,7 +234,7 @@ static int plaquette_st_t(const qcd_lattice *lat, const void *U, double *out_avg
                           cudaStream_t st) {
     const LatP &p = lat->p;
     const int cps = lat->red_chunks_per_seg, nseg = lat->red_nseg;
-    reduce_pass1<T><<<dim3(cps, nseg, 2), RED_THREADS, 0, st>>>(p, -2, 72, U, ws);
+    plaquette_pass1<T><<<dim3(cps, nseg, 2), PLAQ_THREADS, 0, st>>>(p, 1, (const pair_t<T> *)U, ws);
     const int Lt = p.L[3];
     const double Vs = (double)(p.V / Lt);
     if (out_per_t)  // out_per_t[t*2 + comp]
