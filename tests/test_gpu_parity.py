@@ -695,3 +695,18 @@ def test_config_observables_against_stored_oracle_values(qcd, n):
     S1 = beta * 6 * lat.V * (1 - plaq1)
     assert abs(plaq1 - g["plaq1"]) < 1e-12 and abs(K1 - g["K1"]) < 1e-12 * g["K1"]
     assert abs(((K1 + S1) - (K0 + S0)) - g["dH"]) <= 1e-12 * abs(g["K0"] + g["S0"])  # R15: dH against |H|
+
+
+def test_trajectory_driver_reports_the_stored_dH(qcd):
+    """paper_1212_0785_b200.trajectory (per-step observables from the force kernel) on config 2"""
+    import json
+    import os
+    from paper_1212_0785_b200 import trajectory
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "config_values.json")))["2"]
+    r = trajectory.run(2)
+    scale = abs(g["K0"] + g["S0"])
+    assert abs(r["dH"] - g["dH"]) <= 1e-12 * scale and abs(r["dH_from_fused_sums"] - g["dH"]) <= 1e-12 * scale
+    assert abs(r["plaq_end"] - g["plaq1"]) < 1e-12 and len(r["per_step_plaq_K"]) == g["nsteps"]
+    assert abs(r["per_step_plaq_K"][-1][0] - r["plaq_end"]) < 1e-13
+    r2 = trajectory.run(2, observables=False)
+    assert abs(r2["dH"] - r["dH"]) <= 1e-12 * scale
