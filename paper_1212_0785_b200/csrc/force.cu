@@ -522,7 +522,7 @@ static TileP choose_tile(const LatP &lat, int subset, int target, const int *tun
                         double surf = 0;
                         for (int k = 0; k < 4; k++) surf += vol / t[k];
                         // more threads first; then x extent up to 32 (256-byte rows per parity in fp64; measured best on
-                        // B200, profiles/r01b_force_sweeps.md); then compactness
+                        // B200, profiles/r01c_force_sweeps.md); then compactness
                         const double score = threads * 1e6 + (t[0] >= 32 ? 32 : t[0]) * 1e3 - surf / vol * 100.0;
                         if (score > best_score) {
                             best_score = score;
