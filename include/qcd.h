@@ -10,7 +10,7 @@
  * below as O1..O12.
  *
  * CONVENTIONS
- *   Lattice: extents L = (Lx,Ly,Lz,Lt), all even and >= 2, V = Lx*Ly*Lz*Lt < 2^31, periodic.
+ *   Lattice: extents L = (Lx,Ly,Lz,Lt), all even and >= 2, V = Lx*Ly*Lz*Lt < 2^32/36 (119 304 647: 36 V pair indices fit 32 bits), periodic.
  *   Directions mu = 0..3 <-> x,y,z,t.  Lexicographic site index s = x + Lx*(y + Ly*(z + Lz*t)).
  *   parity(s) = (x+y+z+t) & 1;  checkerboard index cb(s) = parity*V/2 + (s>>1).       [O1]
  *
@@ -40,7 +40,7 @@
  *   Return code only: no exceptions, no abort, no printing.  On a nonzero return nothing was
  *   enqueued.  qcd_last_error() returns a thread-local text for the last nonzero return.
  *     QCD_EINVAL      NULL pointer, unknown enum value, nsub < 1, ncomp < 1 ...
- *     QCD_EDIMS       an extent is odd or < 2, or V >= 2^31
+ *     QCD_EDIMS       an extent is odd or < 2, or 36 V >= 2^32
  *     QCD_EALIGN      a field pointer is not 16-byte aligned
  *     QCD_EALIAS      input and output overlap where the operation forbids it
  *     QCD_EWORKSPACE  reserved (workspace too small cannot be detected from a raw pointer)

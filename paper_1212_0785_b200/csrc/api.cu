@@ -71,7 +71,8 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
     for (int d = 0; d < 4; d++) {
         if (dims[d] < 2 || (dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", "qcd_lattice_create");
         V *= dims[d];
-        if (V >= (1ll << 31)) return bad(QCD_EDIMS, "%s: V must be < 2^31", "qcd_lattice_create");
+        // 36 V < 2^32: the kernels index the 36 V complex pairs of a matrix field with 32 bits
+        if (36 * V >= (1ll << 32)) return bad(QCD_EDIMS, "%s: V must be < 2^32 / 36", "qcd_lattice_create");
     }
     qcd_lattice *lat = new (std::nothrow) qcd_lattice;
     if (!lat) return bad(QCD_EINVAL, "%s: out of host memory", "qcd_lattice_create");

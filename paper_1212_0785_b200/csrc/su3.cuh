@@ -29,10 +29,13 @@ template <> __device__ __forceinline__ float rsqrt_<float>(float a) { return 1.0
 
 template <typename T>
 __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
-    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    // 32-bit pair index (36 V < 2^32 is guaranteed by qcd_lattice_create): one IMAD.WIDE per address instead of
+    // 64-bit pointer arithmetic; -10 % instructions in the stencil kernel.  load_link_rw / store_link keep
+    // pointers: with 32-bit indices the link-update kernel needs 173 instead of 156 registers and loses a block.
+    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = __ldg(p + (size_t)e * V);
+        pair_t<T> v = __ldg(f + (i0 + (unsigned)e * (unsigned)V));
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -42,10 +45,10 @@ __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict_
 // reunit() (O9) imposes.  Two thirds of the bytes through L1/L2 for 36 extra FMAs per link.
 template <typename T>
 __device__ __forceinline__ void load_link_su3(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
-    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
 #pragma unroll
     for (int e = 0; e < 6; e++) {
-        pair_t<T> v = __ldg(p + (size_t)e * V);
+        pair_t<T> v = __ldg(f + (i0 + (unsigned)e * (unsigned)V));
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -61,10 +64,10 @@ __device__ __forceinline__ void load_link_su3(M3<T> &m, const pair_t<T> *__restr
 // force kernel), so that it does not displace the neighbour links other threads of the block reuse from L1
 template <typename T>
 __device__ __forceinline__ void load_link_cs(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {
-    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = __ldcs(p + (size_t)e * V);
+        pair_t<T> v = __ldcs(f + (i0 + (unsigned)e * (unsigned)V));
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -72,13 +75,13 @@ __device__ __forceinline__ void load_link_cs(M3<T> &m, const pair_t<T> *f, int V
 
 template <typename T>
 __device__ __forceinline__ void store_link_cs(const M3<T> &m, pair_t<T> *f, int V, int mu, int cb) {
-    pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
 #pragma unroll
     for (int e = 0; e < 9; e++) {
         pair_t<T> v;
         v.x = m.re[e];
         v.y = m.im[e];
-        __stcs(p + (size_t)e * V, v);
+        __stcs(f + (i0 + (unsigned)e * (unsigned)V), v);
     }
 }
 

@@ -47,9 +47,11 @@ def test_lattice_object_and_sizes(qcd):
     big = qcd.Lattice((48, 48, 48, 96))
     assert big.V == 10616832 and big.field_bytes(qcd.F64) == 6115295232
     assert qcd.lib.qcd_version().decode().startswith("qcdmd")
+    assert qcd.Lattice((128, 128, 128, 56)).V == 117440512  # largest class of lattices: 36 V < 2^32
 
 
-@pytest.mark.parametrize("dims", [(3, 4, 4, 4), (4, 4, 4, 1), (0, 2, 2, 2), (2048, 2048, 2048, 2)])
+@pytest.mark.parametrize("dims", [(3, 4, 4, 4), (4, 4, 4, 1), (0, 2, 2, 2), (2048, 2048, 2048, 2),
+                                  (128, 128, 128, 58)])  # the last: V = 121.6 M, 36 V >= 2^32
 def test_bad_extents(qcd, dims):
     with pytest.raises(qcd.QcdError) as e:
         qcd.Lattice(dims)
