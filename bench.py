@@ -296,6 +296,14 @@ def run_ours(args, cfg):
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
                                 "sample": f"{'x'.join(map(str, sd))} lattice with the {cfg['name']} parameters, "
                                           f"5 fused MD steps of the serial C oracle ({dt:.1f} s)"}
+        # the same oracle source built with -fopenmp on all host cores (SURVEY.md 8(d) oracle timing (ii)); extra key
+        omp = Oracle(omp=True)
+        if omp.num_threads() > 1:
+            sd2 = pick_sample(omp, cfg, 6, 10.0)
+            rate2, dt2 = oracle_step_rate(omp, cfg, sd2, 5, 1)
+            line["cpu_baseline_openmp"] = {"value": rate2, "unit": UNIT, "cores": omp.num_threads(), "kind": "oracle",
+                                           "sample": f"{'x'.join(map(str, sd2))} lattice, 5 fused MD steps of the "
+                                                     f"OpenMP build of the same oracle ({dt2:.1f} s)"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
