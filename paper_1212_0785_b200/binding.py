@@ -140,17 +140,33 @@ class Lattice:
     def md_host_work_bytes(self, prec):
         return int(lib.qcd_md_host_work_bytes(self.handle, prec))
 
-    # ---- device memory (PyTorch owns it)
+    # ---- device memory (PyTorch owns it).  Layout of include/qcd.h: chunks of 32 checkerboard sites,
+    # [chunk = cb >> 5][unit][lane = cb & 31]; zero-filled so that the padding of the last chunk is defined
+    @property
+    def nchunks(self):
+        return (self.V + 31) // 32
+
     def new_matrix_field(self, dtype=torch.float64, device="cuda"):
-        """[36][V][2]: entry (mu*9+e, cb, re/im)"""
-        return torch.empty((36, self.V, 2), dtype=dtype, device=device)
+        """[chunk][36][32][2]: entry k = mu*9+e of site cb at [cb >> 5, k, cb & 31, re/im]"""
+        return torch.zeros((self.nchunks, 36, 32, 2), dtype=dtype, device=device)
 
     def new_spinor_field(self, dtype=torch.float64, device="cuda"):
-        """[12][V][2]: spin-colour component k = 3*spin + colour, site cb, re/im"""
-        return torch.empty((12, self.V, 2), dtype=dtype, device=device)
+        """[chunk][12][32][2]: spin-colour component k = 3*spin + colour"""
+        return torch.zeros((self.nchunks, 12, 32, 2), dtype=dtype, device=device)
+
+    def new_pair_field(self, nc, dtype=torch.float64, device="cuda"):
+        """[chunk][nc][32][2]: nc complex units per site (2*nc a multiple of 18 or 24 for qcd_pack)"""
+        return torch.zeros((self.nchunks, nc, 32, 2), dtype=dtype, device=device)
 
     def new_real_field(self, ncomp, dtype=torch.float64, device="cuda"):
-        return torch.empty((ncomp, self.V), dtype=dtype, device=device)
+        """[chunk][ncomp][32]"""
+        return torch.zeros((self.nchunks, ncomp, 32), dtype=dtype, device=device)
+
+    def by_component(self, field):
+        """view-free copy of a device field as [unit][cb] (+ [2] for pair fields): what the layout holds, site by site"""
+        if field.dim() == 4:
+            return field.permute(1, 0, 2, 3).reshape(field.shape[1], -1, 2)[:, :self.V]
+        return field.permute(1, 0, 2).reshape(field.shape[1], -1)[:, :self.V]
 
     def new_workspace(self, device="cuda"):
         return torch.empty(self.workspace_bytes() // 8, dtype=torch.float64, device=device)
@@ -320,6 +336,6 @@ def field_to_device(lat, host_array, dtype=torch.float64):
 
 def field_to_host(lat, dev_field):
     """device matrix field -> numpy complex128 [V,4,3,3]"""
-    t = torch.empty(lat.V * 72, dtype=dev_field.dtype, device=dev_field.device)
+    t = torch.empty(lat.V * 72, dtype=dev_field.dtype, device=dev_field.device)  # canonical: no padding
     qcd_unpack(lat, 72, dev_field, t)
     return t.to(torch.float64).cpu().numpy().view("complex128").reshape(lat.V, 4, 3, 3)

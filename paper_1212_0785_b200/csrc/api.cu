@@ -47,10 +47,13 @@ static int check_ptr(const void *p, const char *fn) {
     if (((uintptr_t)p) & 15) return bad(QCD_EALIGN, "%s: field pointer not 16-byte aligned", fn);
     return QCD_OK;
 }
-static int check_alias(const void *a, const void *b, size_t bytes, const char *fn) {
+static int check_alias2(const void *a, size_t bytes_a, const void *b, size_t bytes_b, const char *fn) {
     const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
-    if (x < y + bytes && y < x + bytes) return bad(QCD_EALIAS, "%s: input and output fields overlap", fn);
+    if (x < y + bytes_b && y < x + bytes_a) return bad(QCD_EALIAS, "%s: input and output fields overlap", fn);
     return QCD_OK;
+}
+static int check_alias(const void *a, const void *b, size_t bytes, const char *fn) {
+    return check_alias2(a, bytes, b, bytes, fn);
 }
 
 }  // namespace qcd
@@ -72,7 +75,7 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
         if (dims[d] < 2 || (dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", "qcd_lattice_create");
         V *= dims[d];
         // 36 V < 2^32: the kernels index the 36 V complex pairs of a matrix field with 32 bits
-        if (36 * V >= (1ll << 32)) return bad(QCD_EDIMS, "%s: V must be < 2^32 / 36", "qcd_lattice_create");
+        if (36 * (V + 32) >= (1ll << 32)) return bad(QCD_EDIMS, "%s: V must be < 2^32 / 36", "qcd_lattice_create");
     }
     qcd_lattice *lat = new (std::nothrow) qcd_lattice;
     if (!lat) return bad(QCD_EINVAL, "%s: out of host memory", "qcd_lattice_create");
@@ -104,7 +107,8 @@ int64_t qcd_lattice_volume(const qcd_lattice *lat) { return lat ? lat->p.V : 0; 
 
 size_t qcd_field_bytes(const qcd_lattice *lat, int prec, int ncomp) {
     if (!lat || ncomp < 1 || (prec != QCD_F32 && prec != QCD_F64)) return 0;
-    return (size_t)lat->p.V * ncomp * real_bytes(prec);
+    const size_t padded = ((size_t)lat->p.V + 31) / 32 * 32;  // whole chunks of 32 sites
+    return padded * ncomp * real_bytes(prec);
 }
 
 size_t qcd_workspace_bytes(const qcd_lattice *lat) { return lat ? lat->workspace_doubles * sizeof(double) : 0; }
@@ -470,7 +474,8 @@ int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, v
     if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
     QCD_TRY(check_ptr(lex_aos, fn));
     QCD_TRY(check_ptr(dev_soa, fn));
-    QCD_TRY(check_alias(lex_aos, dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
+    // the canonical array has exactly V sites, the device field whole chunks of 32
+    QCD_TRY(check_alias2(lex_aos, (size_t)lat->p.V * ncomp * real_bytes(prec), dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
     return launch_pack(lat, prec, ncomp, lex_aos, dev_soa, false, (cudaStream_t)stream);
 }
 
@@ -480,7 +485,7 @@ int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa,
     if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
     QCD_TRY(check_ptr(lex_aos, fn));
     QCD_TRY(check_ptr(dev_soa, fn));
-    QCD_TRY(check_alias(lex_aos, dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
+    QCD_TRY(check_alias2(lex_aos, (size_t)lat->p.V * ncomp * real_bytes(prec), dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
     return launch_pack(lat, prec, ncomp, dev_soa, lex_aos, true, (cudaStream_t)stream);
 }
 
@@ -520,11 +525,12 @@ int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int n
     QCD_TRY(check_ptr(device_work, fn));
     if (nsteps < 0) return bad(QCD_EINVAL, "%s: nsteps < 0", fn);
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    const size_t fb = qcd_field_bytes(lat, prec, 72);                // device field (whole chunks of 32 sites)
+    const size_t hb = (size_t)lat->p.V * 72 * real_bytes(prec);      // canonical host array
     char *w = (char *)device_work;
     void *stageU = w, *stageP = w + fb, *U = w + 2 * fb, *P = w + 3 * fb;
-    cudaError_t e = cudaMemcpyAsync(stageU, U_host, fb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(stageP, P_host, fb, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(stageU, U_host, hb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(stageP, P_host, hb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) {
         set_error("%s: H2D copy: %s", fn, cudaGetErrorString(e));
         return QCD_ECUDA;
@@ -537,8 +543,8 @@ int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int n
     }
     QCD_TRY(launch_pack(lat, prec, 72, U, stageU, true, st));
     QCD_TRY(launch_pack(lat, prec, 72, P, stageP, true, st));
-    e = cudaMemcpyAsync(U_host, stageU, fb, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(P_host, stageP, fb, cudaMemcpyDeviceToHost, st);
+    e = cudaMemcpyAsync(U_host, stageU, hb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P_host, stageP, hb, cudaMemcpyDeviceToHost, st);
     if (e != cudaSuccess) {
         set_error("%s: D2H copy: %s", fn, cudaGetErrorString(e));
         return QCD_ECUDA;

@@ -88,10 +88,10 @@ __global__ void __launch_bounds__(FT_MAX_SITES) force_tile_kernel(const LatP lat
 
     // stage the own links
     {
-        const pair_t<T> *g = U + cb;
+        const pair_t<T> *g = U + unit_index(36, 0, cb);
         pair_t<T> *s = sU + j;
 #pragma unroll 12
-        for (int e = 0; e < 36; e++) s[e * N] = __ldg(g + (size_t)e * V);
+        for (int e = 0; e < 36; e++) s[e * N] = __ldg(g + e * CHUNK);
     }
 
     // neighbour bookkeeping: global index steps, tile-slot steps (within the parity block), in-tile flags

@@ -1,11 +1,13 @@
 // layout.cu — helpers off the hot path: canonical lexicographic AoS <-> device layout, index maps (O1).
 #include "qcd_internal.h"
 #include "site.cuh"
+#include "su3.cuh"
 
 namespace qcd {
 
-// MATRIX layout (ncomp % 18 == 0): real r = 2k+ri of site cb at real index 2*(k*V + cb) + ri.
-// REAL layout: component c of site cb at c*V + cb.
+// Device index of real c of site cb (su3.cuh: chunks of 32 sites).  Pair fields (ncomp a multiple of 18 or 24):
+// unit = complex pair, ncomp/2 units per site, real index 2*unit_index(ncomp/2, c>>1, cb) + (c&1).
+// Real fields: unit = real, ncomp units per site, index unit_index(ncomp, c, cb).
 template <typename T, bool UNPACK>
 __global__ void __launch_bounds__(256) pack_kernel(const LatP lat, const int ncomp, const bool matrix,
                                                    const T *__restrict__ src, T *__restrict__ dst) {
@@ -14,7 +16,7 @@ __global__ void __launch_bounds__(256) pack_kernel(const LatP lat, const int nco
     const Site st = site_of_cb(lat, cb);
     const size_t aos = (size_t)st.s * ncomp;
     for (int c = blockIdx.y; c < ncomp; c += gridDim.y) {
-        const size_t soa = matrix ? 2 * ((size_t)(c >> 1) * lat.V + cb) + (c & 1) : (size_t)c * lat.V + cb;
+        const size_t soa = matrix ? 2 * (size_t)unit_index(ncomp / 2, c >> 1, cb) + (c & 1) : (size_t)unit_index(ncomp, c, cb);
         if (UNPACK) dst[aos + c] = src[soa];
         else dst[soa] = src[aos + c];
     }
@@ -57,7 +59,7 @@ __global__ void __launch_bounds__(256) pack_tr_kernel(const LatP lat, const int 
             const int y = row % lat.L[1], zt = row / lat.L[1];
             const int odd = (y + zt % lat.L[2] + zt / lat.L[2] + par) & 1;
             const int cb = par * lat.Vh + h;
-            const size_t soa = matrix ? 2 * ((size_t)(c >> 1) * lat.V + cb) + (c & 1) : (size_t)c * lat.V + cb;
+            const size_t soa = matrix ? 2 * (size_t)unit_index(ncomp / 2, c >> 1, cb) + (c & 1) : (size_t)unit_index(ncomp, c, cb);
             sm[(2 * hl + odd) * ss + c] = src[soa];
         }
     }
@@ -78,7 +80,7 @@ __global__ void __launch_bounds__(256) pack_tr_kernel(const LatP lat, const int 
             const int y = row % lat.L[1], zt = row / lat.L[1];
             const int odd = (y + zt % lat.L[2] + zt / lat.L[2] + par) & 1;
             const int cb = par * lat.Vh + h;
-            const size_t soa = matrix ? 2 * ((size_t)(c >> 1) * lat.V + cb) + (c & 1) : (size_t)c * lat.V + cb;
+            const size_t soa = matrix ? 2 * (size_t)unit_index(ncomp / 2, c >> 1, cb) + (c & 1) : (size_t)unit_index(ncomp, c, cb);
             dst[soa] = sm[(2 * hl + odd) * ss + c];
         }
 }

@@ -50,21 +50,21 @@ __global__ void __launch_bounds__(128) perturb_kernel(const LatP lat, const uint
     if (cb >= lat.V) return;
     const int mu = blockIdx.y;
     const Site st = site_of_cb(lat, cb);
-    pair_t<T> *p = U + (size_t)(mu * 9) * lat.V + cb;
+    pair_t<T> *p = U + unit_index(36, mu * 9, cb);
 #pragma unroll 1
     for (int e = 0; e < 9; e++) {
         uint32_t w[4];
         double u[2], g[2];
         rng_block(seed, (uint32_t)st.s, (uint32_t)(mu * 16 + e), 0u, 2u, w, u, g);
-        pair_t<T> v = p[(size_t)e * lat.V];
+        pair_t<T> v = p[e * CHUNK];
         v.x = (T)((double)v.x + sigma * g[0]);
         v.y = (T)((double)v.y + sigma * g[1]);
-        p[(size_t)e * lat.V] = v;
+        p[e * CHUNK] = v;
     }
 }
 
 // O15: spin-colour Gaussian fill, component k = blockIdx.y: eta_k(x) = (g0 + i g1)/sqrt(2) of generator block
-// (site, 64 + k, stream_id, purpose 4); pair layout, component k of site cb at pair index k*V + cb
+// (site, 64 + k, stream_id, purpose 4); pair layout with 12 units per site: component k of site cb at unit_index(12, k, cb)
 template <typename T>
 __global__ void __launch_bounds__(128) spinor_gauss_kernel(const LatP lat, const int begin, const int count,
                                                            const uint64_t seed, const uint32_t stream_id,
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(128) spinor_gauss_kernel(const LatP lat, const
     pair_t<T> v;
     v.x = (T)(g[0] * isq2);
     v.y = (T)(g[1] * isq2);
-    out[(size_t)k * lat.V + cb] = v;
+    out[unit_index(12, k, cb)] = v;
 }
 
 int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,

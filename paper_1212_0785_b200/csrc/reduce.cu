@@ -67,12 +67,13 @@ constexpr int SUM_INNER = 3;
 template <typename T>
 __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int V, const T *__restrict__ f, int cb,
                                              const T *__restrict__ f2 = nullptr) {
-    if (kind == QCD_SUM_SCALAR) return (double)__ldg(f + (size_t)comp * V + cb);
+    if (kind == QCD_SUM_SCALAR) return (double)__ldg(f + unit_index(ncomp, comp, cb));
+    const unsigned b0 = unit_index(ncomp / 2, 0, cb);  // pair fields: ncomp/2 complex units per site
     double acc = 0.0;
     if (kind == SUM_INNER) {
         const pair_t<T> *a = (const pair_t<T> *)f, *b = (const pair_t<T> *)f2;
         for (int k = 0; k < ncomp / 2; k++) {
-            const pair_t<T> x = __ldg(a + (size_t)k * V + cb), y = __ldg(b + (size_t)k * V + cb);
+            const pair_t<T> x = __ldg(a + b0 + k * CHUNK), y = __ldg(b + b0 + k * CHUNK);
             if (comp == 0) acc = fma((double)x.x, (double)y.x, fma((double)x.y, (double)y.y, acc));
             else  // both products rounded before the difference (no FMA contraction): Im <a,a> is exactly 0
                 acc += __dsub_rn(__dmul_rn((double)x.x, (double)y.y), __dmul_rn((double)x.y, (double)y.x));
@@ -82,16 +83,16 @@ __device__ __forceinline__ double site_value(int kind, int ncomp, int comp, int 
     if (kind == QCD_SUM_NORM2) {
         const pair_t<T> *p = (const pair_t<T> *)f;
         for (int k = 0; k < ncomp / 2; k++) {
-            const pair_t<T> v = __ldg(p + (size_t)k * V + cb);
+            const pair_t<T> v = __ldg(p + b0 + k * CHUNK);
             acc = fma((double)v.x, (double)v.x, acc);
             acc = fma((double)v.y, (double)v.y, acc);
         }
     } else {
         const pair_t<T> *p = (const pair_t<T> *)f;
         for (int m = 0; m < ncomp / 18; m++) {
-            acc += (double)__ldg(p + (size_t)(m * 9 + 0) * V + cb).x;
-            acc += (double)__ldg(p + (size_t)(m * 9 + 4) * V + cb).x;
-            acc += (double)__ldg(p + (size_t)(m * 9 + 8) * V + cb).x;
+            acc += (double)__ldg(p + b0 + (m * 9 + 0) * CHUNK).x;
+            acc += (double)__ldg(p + b0 + (m * 9 + 4) * CHUNK).x;
+            acc += (double)__ldg(p + b0 + (m * 9 + 8) * CHUNK).x;
         }
     }
     return acc;

@@ -25,17 +25,23 @@ template <typename T> __device__ __forceinline__ T rsqrt_(T a);
 template <> __device__ __forceinline__ double rsqrt_<double>(double a) { return 1.0 / sqrt(a); }
 template <> __device__ __forceinline__ float rsqrt_<float>(float a) { return 1.0f / sqrtf(a); }
 
-// ---- global memory access: entry (mu,e) of site cb at pair index (mu*9+e)*V + cb
+// ---- global memory access.  Device layout (include/qcd.h): array of structures of arrays in chunks of 32
+// checkerboard sites: unit k (of NC per site) of site cb at index ((cb >> 5)*NC + k)*32 + (cb & 31); a matrix
+// field has NC = 36 complex pairs per site, k = mu*9 + e.  A warp reading one entry of 32 consecutive sites reads
+// 512 contiguous bytes (fp64), and all 36 entries of a site sit at compile-time offsets (e*32 units) from one base:
+// one address computation per neighbour site instead of one per load.  36 V < 2^32, so 32-bit indices suffice.
+constexpr int CHUNK = 32;
+
+__host__ __device__ __forceinline__ unsigned unit_index(int NC, int k, int cb) {
+    return ((unsigned)(cb >> 5) * (unsigned)NC + (unsigned)k) * 32u + (unsigned)(cb & 31);
+}
 
 template <typename T>
 __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
-    // 32-bit pair index (36 V < 2^32 is guaranteed by qcd_lattice_create): one IMAD.WIDE per address instead of
-    // 64-bit pointer arithmetic; -10 % instructions in the stencil kernel.  load_link_rw / store_link keep
-    // pointers: with 32-bit indices the link-update kernel needs 173 instead of 156 registers and loses a block.
-    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
+    const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = __ldg(f + (i0 + (unsigned)e * (unsigned)V));
+        pair_t<T> v = __ldg(p + e * CHUNK);
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -45,10 +51,10 @@ __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict_
 // reunit() (O9) imposes.  Two thirds of the bytes through L1/L2 for 36 extra FMAs per link.
 template <typename T>
 __device__ __forceinline__ void load_link_su3(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
-    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
+    const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 6; e++) {
-        pair_t<T> v = __ldg(f + (i0 + (unsigned)e * (unsigned)V));
+        pair_t<T> v = __ldg(p + e * CHUNK);
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -64,10 +70,10 @@ __device__ __forceinline__ void load_link_su3(M3<T> &m, const pair_t<T> *__restr
 // force kernel), so that it does not displace the neighbour links other threads of the block reuse from L1
 template <typename T>
 __device__ __forceinline__ void load_link_cs(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {
-    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
+    const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = __ldcs(f + (i0 + (unsigned)e * (unsigned)V));
+        pair_t<T> v = __ldcs(p + e * CHUNK);
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -75,23 +81,23 @@ __device__ __forceinline__ void load_link_cs(M3<T> &m, const pair_t<T> *f, int V
 
 template <typename T>
 __device__ __forceinline__ void store_link_cs(const M3<T> &m, pair_t<T> *f, int V, int mu, int cb) {
-    const unsigned i0 = (unsigned)(mu * 9) * (unsigned)V + (unsigned)cb;
+    pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
         pair_t<T> v;
         v.x = m.re[e];
         v.y = m.im[e];
-        __stcs(f + (i0 + (unsigned)e * (unsigned)V), v);
+        __stcs(p + e * CHUNK, v);
     }
 }
 
 // same, through the normal (coherent) path: for fields the kernel also writes
 template <typename T>
 __device__ __forceinline__ void load_link_rw(M3<T> &m, const pair_t<T> *f, int V, int mu, int cb) {
-    const pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = p[(size_t)e * V];
+        pair_t<T> v = p[e * CHUNK];
         m.re[e] = v.x;
         m.im[e] = v.y;
     }
@@ -99,13 +105,13 @@ __device__ __forceinline__ void load_link_rw(M3<T> &m, const pair_t<T> *f, int V
 
 template <typename T>
 __device__ __forceinline__ void store_link(const M3<T> &m, pair_t<T> *f, int V, int mu, int cb) {
-    pair_t<T> *p = f + (size_t)(mu * 9) * V + cb;
+    pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
         pair_t<T> v;
         v.x = m.re[e];
         v.y = m.im[e];
-        p[(size_t)e * V] = v;
+        p[e * CHUNK] = v;
     }
 }
 

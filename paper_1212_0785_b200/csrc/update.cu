@@ -39,18 +39,18 @@ __global__ void __launch_bounds__(256) mom_update_kernel(const int V, const int 
                                                          const pair_t<T> *__restrict__ F, pair_t<T> *__restrict__ P) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
-    const size_t base = (size_t)(blockIdx.y * 9) * V + begin + i;
+    const unsigned base = unit_index(36, blockIdx.y * 9, begin + i);
     pair_t<T> f[9], p[9];
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        f[e] = __ldg(F + base + (size_t)e * V);
-        p[e] = P[base + (size_t)e * V];
+        f[e] = __ldg(F + base + e * CHUNK);
+        p[e] = P[base + e * CHUNK];
     }
 #pragma unroll
     for (int e = 0; e < 9; e++) {
         p[e].x = fma_(eps, f[e].x, p[e].x);
         p[e].y = fma_(eps, f[e].y, p[e].y);
-        P[base + (size_t)e * V] = p[e];
+        P[base + e * CHUNK] = p[e];
     }
 }
 

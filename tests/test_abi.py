@@ -46,6 +46,10 @@ def test_lattice_object_and_sizes(qcd):
     assert lat.md_host_work_bytes(qcd.F64) == 4 * lat.field_bytes(qcd.F64)
     big = qcd.Lattice((48, 48, 48, 96))
     assert big.V == 10616832 and big.field_bytes(qcd.F64) == 6115295232
+    # fields are whole chunks of 32 sites: V = 16 occupies one chunk, V = 480 fifteen
+    assert qcd.Lattice((2, 2, 2, 2)).field_bytes(qcd.F64) == 32 * 72 * 8
+    assert qcd.Lattice((4, 10, 6, 2)).field_bytes(qcd.F32, 24) == 480 * 24 * 4
+    assert qcd.Lattice((2, 2, 2, 6)).field_bytes(qcd.F64) == 64 * 72 * 8  # V = 48 -> two chunks
     assert qcd.lib.qcd_version().decode().startswith("qcdmd")
     assert qcd.Lattice((128, 128, 128, 56)).V == 117440512  # largest class of lattices: 36 V < 2^32
 

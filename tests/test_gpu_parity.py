@@ -106,9 +106,14 @@ def test_pack_unpack_layout(qcd, orc, prec, dims):
     A = round_to(prec, inputs.random_matrix_field(3, V))
     d = dev(qcd, lat, A, prec)
     assert np.array_equal(host(qcd, lat, d), A)  # round trip is exact
-    # documented layout: pair (mu*9+e) of site cb at pair index (mu*9+e)*V + cb
-    raw = d.cpu().numpy().astype(np.float64)  # [36][V][2]
+    # documented layout: pair k = mu*9+e of site cb at [cb >> 5][k][cb & 31] (chunks of 32 checkerboard sites)
+    assert tuple(d.shape) == ((V + 31) // 32, 36, 32, 2) and d.numel() * d.element_size() == lat.field_bytes(
+        qcd.F64 if prec == "f64" else qcd.F32)
+    raw4 = d.cpu().numpy().astype(np.float64)
     cb = orc.map(dims, O.MAP_CB_OF_LEX)
+    k_probe, s_probe = 17, V - 1  # one element by the index formula itself
+    assert raw4[cb[s_probe] >> 5, k_probe, cb[s_probe] & 31, 0] == A.reshape(V, 36)[s_probe, k_probe].real
+    raw = lat.by_component(d).cpu().numpy().astype(np.float64)  # [36][V][2] by checkerboard index
     ref = np.empty((36, V, 2))
     flat = A.reshape(V, 36)
     ref[:, cb, 0] = flat.real.T
@@ -119,7 +124,7 @@ def test_pack_unpack_layout(qcd, orc, prec, dims):
     src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
     dst = lat.new_real_field(3, tdtype(prec))
     qcd.qcd_pack(lat, 3, src, dst)
-    got = dst.cpu().numpy().astype(np.float64)
+    got = lat.by_component(dst).cpu().numpy().astype(np.float64)
     assert np.array_equal(got[:, cb], R.T)
     back = torch.empty_like(src)
     qcd.qcd_unpack(lat, 3, dst, back)
@@ -129,7 +134,7 @@ def test_pack_unpack_layout(qcd, orc, prec, dims):
     src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
     dst = lat.new_real_field(100, tdtype(prec))
     qcd.qcd_pack(lat, 100, src, dst)
-    assert np.array_equal(dst.cpu().numpy().astype(np.float64)[:, cb], R.T)
+    assert np.array_equal(lat.by_component(dst).cpu().numpy().astype(np.float64)[:, cb], R.T)
     back = torch.empty_like(src)
     qcd.qcd_unpack(lat, 100, dst, back)
     assert torch.equal(back, src)
@@ -573,8 +578,8 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
     cbmap = orc_omp.map(dims, O.MAP_CB_OF_LEX)
     cbs = torch.from_numpy(cbmap[sites].astype(np.int64)).cuda()
 
-    def gather(field):  # device field [36][V][2] -> complex [n,4,3,3] at the sampled sites
-        g = field[:, cbs, :].to(torch.float64).cpu().numpy()
+    def gather(field):  # device field [chunk][36][32][2] -> complex [n,4,3,3] at the sampled sites
+        g = field[cbs >> 5, :, cbs & 31, :].permute(1, 0, 2).to(torch.float64).cpu().numpy()
         return (g[..., 0] + 1j * g[..., 1]).T.reshape(len(sites), 4, 3, 3)
 
     tolgen = 1e-12 if prec == "f64" else 2e-7

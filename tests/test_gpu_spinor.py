@@ -21,14 +21,14 @@ def qcd():
 def spinor_to_device(qcd, lat, a, prec):
     import torch
     t = torch.view_as_real(torch.from_numpy(np.ascontiguousarray(a))).reshape(-1).to(tdtype(prec)).cuda()
-    out = torch.empty((a.shape[1], lat.V, 2), dtype=tdtype(prec), device="cuda")
+    out = lat.new_pair_field(a.shape[1], tdtype(prec))
     qcd.qcd_pack(lat, 2 * a.shape[1], t, out)
     return out
 
 
 def spinor_to_host(qcd, lat, d):
     import torch
-    nc = d.shape[0]
+    nc = d.shape[1]
     t = torch.empty(lat.V * nc * 2, dtype=d.dtype, device="cuda")
     qcd.qcd_unpack(lat, 2 * nc, d, t)
     return t.to(torch.float64).cpu().numpy().view("complex128").reshape(lat.V, nc)
@@ -53,10 +53,10 @@ def test_spinor_gaussian(qcd, orc_omp, prec, dims):
         g = spinor_to_host(qcd, lat, eta)
         assert np.abs(g[par == p] - ref[par == p]).max() < tol * np.abs(ref).max()
         assert np.all(g[par != p] == 7.0 + 7.0j)
-    # layout: component k of checkerboard site cb at pair index k*V + cb
+    # layout: component k of checkerboard site cb at [cb >> 5][k][cb & 31]
     cb = orc_omp.map(dims, O.MAP_CB_OF_LEX)
     qcd.qcd_spinor_gaussian(lat, eta, seed, stream_id=3)
-    raw = eta.to("cpu").numpy().astype(np.float64)
+    raw = lat.by_component(eta).to("cpu").numpy().astype(np.float64)
     assert np.abs(raw[5, cb, 0] - ref[:, 5].real).max() < tol * 5 and np.abs(raw[11, cb, 1] - ref[:, 11].imag).max() < tol * 5
 
 
