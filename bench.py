@@ -3,10 +3,13 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
 
-A "step" is one fused molecular-dynamics step on the whole lattice: qcd_force_mom_update
-(P += eps F(U)) then qcd_link_update with reunit (U <- reunit(exp(i eps P) U)) — both kernels of
-SURVEY.md section 8(a)'s "MD step (fused)" row.  Default workload: BASELINE config 4, 32^3x64 fp64,
-sigma=0.2, beta=6.0, eps=0.02, seeded synthetic hot start generated on the device.
+A "step" is one fused molecular-dynamics step on the whole lattice: P += eps F(U), then
+U <- reunit(exp(i eps P) U) — force, projection, momentum update, exponential, link update and
+reunitarisation, all rows of SURVEY.md section 8(a)'s MD step.  --path single_pass (default, the faster one as
+measured: profiles/r01d_*.md) runs it as ONE kernel, qcd_md_step_single_pass, ping-ponging two gauge fields
+(8(a) "MD step (single pass)", 288 reals/site); --path two_kernel as qcd_force_mom_update followed by
+qcd_link_update(reunit) in place (8(a) "MD step (fused)", 432 reals/site).  Default workload: BASELINE
+config 4, 32^3x64 fp64, sigma=0.2, beta=6.0, eps=0.02, seeded synthetic hot start generated on the device.
 
 N > 1 (torchrun): the path is run as N independent replicas (one lattice per GPU, different seeds,
 no data-path collective); value = total site-updates/s, scaling "weak".
@@ -408,9 +411,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--path", default="two_kernel", choices=["two_kernel", "single_pass"],
-                    help="two_kernel: qcd_force_mom_update + qcd_link_update(reunit) in place (default, the faster "
-                         "one as measured); single_pass: qcd_md_step_single_pass ping-ponging two gauge fields")
+    ap.add_argument("--path", default="single_pass", choices=["two_kernel", "single_pass"],
+                    help="single_pass (default, the faster one as measured): qcd_md_step_single_pass ping-ponging two "
+                         "gauge fields; two_kernel: qcd_force_mom_update + qcd_link_update(reunit) in place")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-kernel", action="store_true",

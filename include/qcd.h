@@ -17,11 +17,16 @@
  *   Precision `prec`: QCD_F64 fields are double, QCD_F32 fields are float.  All field arithmetic is
  *   done in the field's precision; every reduction accumulates and returns double.
  *
- *   DEVICE layout of a matrix field (U, P, F; 4 links per site, 3x3 complex each = 72 reals/site):
- *   checkerboarded, site-fastest structure of arrays of complex pairs.  Entry (mu, e = 3*row+col)
- *   of site cb is the (re,im) pair at pair-index (mu*9 + e)*V + cb, i.e. a `double2`/`float2`
- *   array of 36*V pairs.  Even sites are cb in [0,V/2), odd sites [V/2,V).
- *   DEVICE layout of a real site field with ncomp components: real index comp*V + cb.
+ *   DEVICE layout: checkerboarded, site-fastest arrays in CHUNKS OF 32 SITES.  A field with NC units per
+ *   site (a unit is a (re,im) pair = `double2`/`float2` for matrix, spin-colour and other pair fields, one
+ *   real for real fields) stores unit k of checkerboard site cb at unit index
+ *       ((cb >> 5)*NC + k)*32 + (cb & 31)            i.e. [chunk = cb/32][k][lane = cb%32].
+ *   Matrix fields (U, P, F; 4 links per site, 3x3 complex each = 72 reals/site): NC = 36, k = mu*9 + e,
+ *   e = 3*row + col.  A warp reading one entry of 32 consecutive sites reads 512 contiguous bytes (fp64), and
+ *   the 36 entries of a site sit at fixed offsets (k*32 units) from the site's base address.  Even sites
+ *   are cb in [0,V/2), odd sites [V/2,V).  A field occupies whole chunks: qcd_field_bytes rounds V up to a
+ *   multiple of 32 sites; the padding is never read or written.
+ *   Real site fields with ncomp components: NC = ncomp, unit = one real.
  *   CANONICAL (exchange) layout, used by qcd_pack/qcd_unpack and the *_host call: lexicographic
  *   array of structures [s][mu][row][col][re,im] (matrix) or [s][comp] (real).
  *
@@ -214,7 +219,7 @@ int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2]
  * Only the site-parallel pieces outside the Dirac operator (which, with the solver, is out of scope:
  * PAPER.md:83): Gaussian fill of a spin-colour vector field and its norm / inner-product reductions
  * (PAPER.md:26).  A spin-colour vector has 12 complex components per site, k = 3*spin + colour; device
- * layout: complex pairs, component k of checkerboard site cb at pair index k*V + cb (24 reals per site;
+ * layout: complex pairs, NC = 12 units per site, component k of site cb at unit index ((cb>>5)*12 + k)*32 + (cb&31) (24 reals per site;
  * qcd_pack / qcd_unpack use this pair layout whenever ncomp is a multiple of 18 or of 24; canonical
  * layout [s][k][re,im]).  [O15] eta_k(x) = (g0 + i g1)/sqrt(2), (g0,g1) the Box-Muller pair of generator
  * block (lexicographic site, 64 + k, stream_id, purpose 4): <|eta_k|^2> = 1, weight exp(-eta^dag eta).
@@ -257,8 +262,9 @@ int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int 
 
 /* ---- helpers (not on the hot path) -------------------------------------------------------- */
 
-/* canonical lexicographic AoS (device) -> device layout, and back. ncomp reals per site, even. For
- * matrix fields ncomp = 72.  Input and output must not overlap. */
+/* canonical lexicographic AoS (device, exactly V*ncomp reals) -> device layout (qcd_field_bytes bytes), and back.
+ * ncomp reals per site; ncomp a multiple of 18 or 24 selects the pair layout (NC = ncomp/2), any other ncomp
+ * the real layout (NC = ncomp).  For matrix fields ncomp = 72.  Input and output must not overlap. */
 int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream);
 int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa, void *lex_aos, void *stream);
 /* index / subset maps [O1] into dev_out (int32[V]) */
