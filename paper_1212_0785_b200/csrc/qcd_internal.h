@@ -1,7 +1,7 @@
 // qcd_internal.h — host/device shared declarations of libqcdmd (not part of the public ABI).
 //
-// Device layout (include/qcd.h): a matrix field is an array of 36*V complex pairs; entry
-// (mu, e=3*row+col) of checkerboard site cb sits at pair index (mu*9+e)*V + cb.
+// Device layout (include/qcd.h, su3.cuh): chunks of 32 checkerboard sites; unit k (of NC per site) of site cb at
+// ((cb >> 5)*NC + k)*32 + (cb & 31); a matrix field has NC = 36 complex pairs per site, k = mu*9 + 3*row + col.
 #pragma once
 
 #include <cuda_runtime.h>
