@@ -245,6 +245,12 @@ __device__ __forceinline__ void reunit(M3<T> &M) {
 // (iQ)^k / k! = a_k + b_k Q + c_k Q^2 with (a,b,c)_{k+1} = (i/(k+1)) (c0 c_k, a_k + c1 c_k, b_k).
 // Q is first scaled by 2^-n so that ||Q||_F <= 1 (series terms decay from the start: no
 // cancellation), the result squared n times.  NT = number of series terms kept.
+// 1/k, k = 0..23 (entry 0 unused), correctly rounded doubles
+__device__ __constant__ const double c_inv_k[24] = {0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8,
+                                                    1.0 / 9, 1.0 / 10, 1.0 / 11, 1.0 / 12, 1.0 / 13, 1.0 / 14, 1.0 / 15,
+                                                    1.0 / 16, 1.0 / 17, 1.0 / 18, 1.0 / 19, 1.0 / 20, 1.0 / 21, 1.0 / 22,
+                                                    1.0 / 23};
+
 template <typename T> struct ExpTerms;
 template <> struct ExpTerms<double> { static constexpr int max_terms = 22; static constexpr double tol = 1e-18; };
 template <> struct ExpTerms<float> { static constexpr int max_terms = 13; static constexpr float tol = 1e-9f; };
@@ -286,7 +292,7 @@ __device__ __forceinline__ void expi_herm(M3<T> &E, const M3<T> &Qin) {
     // bound on the k-th term: x^k/k! with x = ||Q||_F <= 1
     T x = sqrt(n2), bound = T(1);
     for (int k = 1; k <= ExpTerms<T>::max_terms; k++) {
-        const T inv = T(1) / T(k);
+        const T inv = (T)c_inv_k[k];  // 1/k from a table: an fp64 division is a dozen instructions
         // (a,b,c) <- (i/k) (c0 c, a + c1 c, b);  i (x + i y) = -y + i x
         const T tar = c0 * cr, tai = c0 * ci;
         const T tbr = fma_(c1, cr, ar), tbi = fma_(c1, ci, ai);
