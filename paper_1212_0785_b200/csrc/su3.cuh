@@ -22,8 +22,8 @@ template <> __device__ __forceinline__ double fma_<double>(double a, double b, d
 template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
 
 template <typename T> __device__ __forceinline__ T rsqrt_(T a);
-template <> __device__ __forceinline__ double rsqrt_<double>(double a) { return 1.0 / sqrt(a); }
-template <> __device__ __forceinline__ float rsqrt_<float>(float a) { return 1.0f / sqrtf(a); }
+template <> __device__ __forceinline__ double rsqrt_<double>(double a) { return rsqrt(a); }  // <= 1 ulp
+template <> __device__ __forceinline__ float rsqrt_<float>(float a) { return rsqrtf(a); }
 
 // ---- global memory access.  Device layout (include/qcd.h): array of structures of arrays in chunks of 32
 // checkerboard sites: unit k (of NC per site) of site cb at index ((cb >> 5)*NC + k)*32 + (cb & 31); a matrix
