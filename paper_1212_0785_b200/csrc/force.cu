@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(NT, MINB) force_kernel(const LatP lat, const T
                 }
                 M3<T> E, R;
                 expi_herm(E, P);
-                mul<false, false, false>(R, E, Um);
+                mul_top2(R, E, Um);  // reunit rebuilds row 2
                 reunit(R);
                 store_link_cs(R, Uout, V, mu, cb);
             }

@@ -141,6 +141,29 @@ __device__ __forceinline__ void mul(M3<T> &C, const M3<T> &A, const M3<T> &B) {
         }
 }
 
+// rows 0 and 1 of C = A B only (row 2 of C is left untouched): what reunit() needs of exp(i eps P) U, since it
+// rebuilds the third row from the first two
+template <typename T>
+__device__ __forceinline__ void mul_top2(M3<T> &C, const M3<T> &A, const M3<T> &B) {
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            T cr = T(0), ci = T(0);
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                const T ar = A.re[3 * i + k], ai = A.im[3 * i + k];
+                const T br = B.re[3 * k + j], bi = B.im[3 * k + j];
+                cr = fma_(ar, br, cr);
+                cr = fma_(-ai, bi, cr);
+                ci = fma_(ar, bi, ci);
+                ci = fma_(ai, br, ci);
+            }
+            C.re[3 * i + j] = cr;
+            C.im[3 * i + j] = ci;
+        }
+}
+
 // Re tr (A B^dagger) = sum_ij Re(A_ij conj(B_ij))
 template <typename T>
 __device__ __forceinline__ T retr_mul_dag(const M3<T> &A, const M3<T> &B) {

@@ -28,7 +28,8 @@ __global__ void __launch_bounds__(256) link_update_kernel(const int V, const int
             Q.im[e] *= eps;
         }
         expi_herm(E, Q);
-        mul<false, false, false>(R, E, Ul);
+        if (MODE == 1) mul_top2(R, E, Ul);  // reunit rebuilds row 2
+        else mul<false, false, false>(R, E, Ul);
     }
     if (MODE >= 1) reunit(R);
     store_link(R, U, V, mu, cb);
