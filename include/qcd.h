@@ -240,15 +240,18 @@ int qcd_inner_product_multi(const qcd_lattice *lat, int prec, int nc, const void
  * database.  Here the measuring lives in paper_1212_0785_b200/autotune.py (it calls the public kernels);
  * these calls are the database the launchers consult.  Key: (lattice extents, prec, subset ALL or
  * EVEN/ODD, kernel).  Value: for QCD_KERNEL_FORCE a kernel variant and a 4-D block tile (tile[0] = 0 or
- * tile = NULL: the library's own choice; extents must divide the lattice, tile[0] even, and the block must
- * not exceed the variant's thread limit: 128 sites for SITE, 256 for SITE256/PIPE/PLANE, 128 for LINK);
- * for QCD_KERNEL_LINK_UPDATE / QCD_KERNEL_MOM_UPDATE the threads per block (multiple of 32, 32..256).
- * Environment variables QCD_FORCE_VARIANT / QCD_TILE, when set, still win (sweeps).  Results never depend
- * on these settings beyond rounding order; reductions are not tunable (fixed geometry, determinism).
- * Host-only, thread-safe, process-global.  qcd_tune_get returns QCD_EINVAL when no entry exists. */
+ * tile = NULL: the library's own choice; extents must divide the lattice, tile[0] even, at most 128 sites of
+ * the subset per block); for QCD_KERNEL_LINK_UPDATE / QCD_KERNEL_MOM_UPDATE the threads per block (multiple
+ * of 32, 32..256).  The database is the only knob: no environment variable is read.  Both force variants
+ * compute the definition [O7] for arbitrary 3x3 matrices; results never depend on these settings beyond
+ * rounding order; reductions are not tunable (fixed geometry, determinism).
+ * Host-only, thread-safe, process-global.  qcd_tune_get returns QCD_EINVAL when no entry exists.
+ *   QCD_FORCE_STAPLE  the definition as written: per direction 6 staples of 2 products, then U_mu(x) A
+ *                     (52 products, 76 link loads per site)
+ *   QCD_FORCE_PLANE   (default) every plane visited once, its closed plaquette shared by the two directions
+ *                     (46 products, 64 link loads per site) */
 enum { QCD_KERNEL_FORCE = 0, QCD_KERNEL_LINK_UPDATE = 1, QCD_KERNEL_MOM_UPDATE = 2 };
-enum { QCD_FORCE_SITE = 0, QCD_FORCE_SITE256 = 1, QCD_FORCE_PIPE = 2, QCD_FORCE_PLANE = 3, QCD_FORCE_LINK = 4,
-       QCD_FORCE_TILE = 5, QCD_FORCE_PLAQ = 6 };
+enum { QCD_FORCE_STAPLE = 0, QCD_FORCE_PLANE = 1 };
 int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int variant, const int tile[4],
                  int threads);
 int qcd_tune_get(const qcd_lattice *lat, int prec, int subset, int kernel, int *variant, int tile[4],

@@ -14,7 +14,6 @@ JSON and loaded again later (`load`).  Only launch parameters change; results st
 import argparse
 import itertools
 import json
-import os
 import sys
 
 import torch
@@ -22,8 +21,8 @@ import torch
 from . import binding as qcd
 
 SITE_LOCAL_THREADS = (32, 64, 96, 128, 160, 192, 224, 256)
-FORCE_BLOCK_LIMIT = {"site": 128, "site256": 256, "pipe": 256, "plane": 256, "link": 128}
-FORCE_VARIANTS = ("site", "site256", "plane", "pipe", "link")
+FORCE_BLOCK_SITES = 128  # threads per block of the stencil kernels (one thread per site of the subset)
+FORCE_VARIANTS = ("plane", "staple")
 
 
 def _divisors(n, even=False):
@@ -62,9 +61,6 @@ def _time(fn, warm=3, reps=10):
 def tune(dims, dtype=torch.float64, subset=qcd.ALL, beta=6.0, eps=0.02, sigma=0.2, reps=10, verbose=True):
     """measure every candidate for the three tunable kernels on lattice `dims`; set the winners in the library;
     return the table (list of dict entries, one per kernel)"""
-    for k in list(os.environ):  # environment overrides would defeat the database
-        if k in ("QCD_FORCE_VARIANT", "QCD_TILE"):
-            del os.environ[k]
     prec = qcd.F64 if dtype == torch.float64 else qcd.F32
     lat = qcd.Lattice(dims)
     U, P, F = lat.new_matrix_field(dtype), lat.new_matrix_field(dtype), lat.new_matrix_field(dtype)
@@ -86,7 +82,7 @@ def tune(dims, dtype=torch.float64, subset=qcd.ALL, beta=6.0, eps=0.02, sigma=0.
     cands = []
     for v in FORCE_VARIANTS:
         npar = 2 if subset == qcd.ALL else 1
-        for tile in force_tiles(dims, FORCE_BLOCK_LIMIT[v] * 2 // npar):
+        for tile in force_tiles(dims, FORCE_BLOCK_SITES * 2 // npar):
             try:
                 qcd.qcd_tune_set(lat, prec, subset, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index(v), tile)
             except qcd.QcdError:

@@ -17,7 +17,7 @@ ALL, EVEN, ODD = 0, 1, 2
 SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
 OK, EINVAL, EDIMS, EALIGN, EALIAS, EWORKSPACE, ECUDA = range(7)
 KERNEL_FORCE, KERNEL_LINK_UPDATE, KERNEL_MOM_UPDATE = 0, 1, 2
-FORCE_VARIANTS = ("site", "site256", "pipe", "plane", "link", "tile", "plaq")  # index = QCD_FORCE_* value
+FORCE_VARIANTS = ("staple", "plane")  # index = QCD_FORCE_* value
 MAP_CB_OF_LEX, MAP_LEX_OF_CB, MAP_NBR_FWD0, MAP_NBR_BWD0, MAP_PARITY, MAP_TSLICE = 0, 1, 2, 6, 10, 11
 
 # every symbol include/qcd.h declares, with its ctypes signature (restype, argtypes)

@@ -94,6 +94,8 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
     const size_t b = (size_t)MAX_NSUB * RED_GENERIC_CHUNKS;
     const size_t c = 2 * ((size_t)V / 32 + 1);  // per-block partial pairs of the kernels that reduce as a by-product
     lat->workspace_doubles = (a > b ? (a > c ? a : c) : (b > c ? b : c)) + 64;
+    default_force_tile(lat->p, 2, lat->tile_all);
+    default_force_tile(lat->p, 1, lat->tile_par);
     *out = lat;
     return QCD_OK;
 }
@@ -259,7 +261,7 @@ int qcd_force_mom_update_sums(const qcd_lattice *lat, int prec, double beta, dou
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
-    return launch_force_sums(lat, prec, beta, eps, U, P, out, (double *)workspace, (cudaStream_t)stream);
+    return launch_force_sums(lat, prec, beta, eps, 0.0, U, P, nullptr, out, (double *)workspace, (cudaStream_t)stream);
 }
 
 int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
@@ -277,7 +279,7 @@ int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double ep
         QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
         if (k < nsteps - 1) QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps, U, P, true, st));
     }
-    return launch_force_sums(lat, prec, beta, 0.5 * eps, U, P, out, (double *)workspace, st);
+    return launch_force_sums(lat, prec, beta, 0.5 * eps, 0.0, U, P, nullptr, out, (double *)workspace, st);
 }
 
 int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
@@ -425,7 +427,7 @@ int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int v
     QCD_TRY(check_subset(subset, fn));
     TuneCfg cfg = {0, {0, 0, 0, 0}, 0};
     if (kernel == QCD_KERNEL_FORCE) {
-        if (variant < QCD_FORCE_SITE || variant > QCD_FORCE_PLAQ) return bad(QCD_EINVAL, "%s: unknown force variant", fn);
+        if (variant != QCD_FORCE_STAPLE && variant != QCD_FORCE_PLANE) return bad(QCD_EINVAL, "%s: unknown force variant", fn);
         cfg.variant = variant;
         if (tile && tile[0]) {
             long sites = 1;
@@ -436,9 +438,7 @@ int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int v
             }
             if (tile[0] & 1) return bad(QCD_EINVAL, "%s: tile[0] must be even", fn);
             const long threads_needed = subset == QCD_ALL ? sites : sites / 2;
-            const long limit = variant == QCD_FORCE_SITE || variant == QCD_FORCE_LINK ? 128 : 256;
-            if (variant <= QCD_FORCE_LINK && threads_needed > limit)
-                return bad(QCD_EINVAL, "%s: tile has more sites than the variant's block can hold", fn);
+            if (threads_needed > 128) return bad(QCD_EINVAL, "%s: tile has more sites than a block can hold (128)", fn);
         }
     } else if (kernel == QCD_KERNEL_LINK_UPDATE || kernel == QCD_KERNEL_MOM_UPDATE) {
         if (threads < 32 || threads > 256 || threads % 32) return bad(QCD_EINVAL, "%s: threads must be 32..256, multiple of 32", fn);

@@ -43,6 +43,8 @@ struct qcd_lattice {
     int red_chunks_per_seg;  // first-pass blocks per (timeslice, parity) segment
     int red_nseg;            // 2*Lt segments
     size_t workspace_doubles;
+    int tile_all[4];  // default 4-D block tile of the stencil kernel, subset ALL (both parities per block)
+    int tile_par[4];  // the same for one parity (EVEN / ODD)
 };
 
 namespace qcd {
@@ -73,12 +75,8 @@ int launch_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double 
 // single-pass MD step (force.cu): P += eps_p F(U); Uout = reunit(exp(i eps_u P) U); U and Uout distinct
 int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
                      void *Uout, cudaStream_t st);
-// plaquette-sharing force kernel (force_plaq.cu): subset ALL, unitary links
-int launch_gauge_force_plaq(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *out,
-                            bool fused_mom, cudaStream_t st);
-// staple kernel with the tile's own links staged in shared memory (force_tile.cu): subset ALL; -1 = not applicable
-int launch_gauge_force_tile(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *out,
-                            bool fused_mom, cudaStream_t st);
+// default block tile of the stencil kernels (force.cu), computed once per lattice
+void default_force_tile(const LatP &lat, int npar, int out[4]);
 int launch_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P,
                       cudaStream_t st);
 int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,
@@ -95,9 +93,10 @@ int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp
                double *ws, cudaStream_t st);
 int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,
                      const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st);
-// force + momentum update with plaquette and kinetic-energy sums as by-products (force.cu); ws: 2*blocks doubles
-int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P, double *out,
-                      double *ws, cudaStream_t st);
+// force + momentum update (+ link update into Uout when Uout != NULL: the single-pass step) with plaquette and
+// kinetic-energy sums as by-products (force.cu); ws: 2*blocks doubles
+int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
+                      void *Uout, double *out, double *ws, cudaStream_t st);
 int launch_sum_partials(const double *partial, int count, double scale, double *out, cudaStream_t st);
 int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
                            cudaStream_t st);

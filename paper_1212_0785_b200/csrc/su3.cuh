@@ -278,74 +278,118 @@ template <typename T> struct ExpTerms;
 template <> struct ExpTerms<double> { static constexpr int max_terms = 22; static constexpr double tol = 1e-18; };
 template <> struct ExpTerms<float> { static constexpr int max_terms = 13; static constexpr float tol = 1e-9f; };
 
-template <typename T>
-__device__ __forceinline__ void expi_herm(M3<T> &E, const M3<T> &Qin) {
+// E = exp(i eps P) for Hermitian traceless P; only the upper triangle of P is read (P_ji = conj P_ij).
+// ROWS = 2: only rows 0 and 1 of E are formed (what reunit() needs of exp(i eps P) U, since it rebuilds the third
+// row); ROWS = 3: all of E.
+// Arithmetic per link: Q^2 is Hermitian (6 entries, 54 FMAs instead of 108); the series runs on REAL
+// coefficients — Q^k/k! = al_k + be_k Q + ga_k Q^2 with (al,be,ga)_{k+1} = (c0 ga, al + c1 ga, be)/(k+1), and
+// i^k only decides whether a term adds to the real or the imaginary part of f0, f1, f2 and with which sign.
+template <int ROWS, typename T>
+__device__ __forceinline__ void expi_herm_scaled(M3<T> &E, const M3<T> &P, const T eps) {
+    // ||eps P||_F^2 from the upper triangle
     T n2 = T(0);
 #pragma unroll
-    for (int e = 0; e < 9; e++) n2 = fma_(Qin.re[e], Qin.re[e], fma_(Qin.im[e], Qin.im[e], n2));
+    for (int i = 0; i < 3; i++) n2 = fma_(P.re[4 * i], P.re[4 * i], n2);
+    T off = T(0);
+    const int I[3] = {0, 0, 1}, J[3] = {1, 2, 2};
+#pragma unroll
+    for (int p = 0; p < 3; p++) {
+        const int e = 3 * I[p] + J[p];
+        off = fma_(P.re[e], P.re[e], fma_(P.im[e], P.im[e], off));
+    }
+    n2 = fma_(T(2), off, n2) * eps * eps;
     int nsq = 0;
-    T scale = T(1);
-    while (n2 * scale * scale > T(1)) {
+    T scale = eps;
+    while (n2 > T(1)) {
         scale *= T(0.5);
+        n2 *= T(0.25);
         nsq++;
     }
-    M3<T> Q;
+    // Q = scale * P: d[i] = Q_ii (real), (xr, xi)[p] = Q_ij for (ij) = (01), (02), (12)
+    T d[3], xr[3], xi[3];
 #pragma unroll
-    for (int e = 0; e < 9; e++) {
-        Q.re[e] = Qin.re[e] * scale;
-        Q.im[e] = Qin.im[e] * scale;
+    for (int i = 0; i < 3; i++) d[i] = P.re[4 * i] * scale;
+#pragma unroll
+    for (int p = 0; p < 3; p++) {
+        xr[p] = P.re[3 * I[p] + J[p]] * scale;
+        xi[p] = P.im[3 * I[p] + J[p]] * scale;
     }
-    n2 *= scale * scale;
-    M3<T> Q2;
-    mul<false, false, false>(Q2, Q, Q);
+    // Q2 = Q Q, Hermitian: D[i] = sum_k |Q_ik|^2; (Xr, Xi)[p] = sum_k Q_ik Q_kj
+    const T a01 = fma_(xr[0], xr[0], xi[0] * xi[0]);
+    const T a02 = fma_(xr[1], xr[1], xi[1] * xi[1]);
+    const T a12 = fma_(xr[2], xr[2], xi[2] * xi[2]);
+    T D[3], Xr[3], Xi[3];
+    D[0] = fma_(d[0], d[0], a01 + a02);
+    D[1] = fma_(d[1], d[1], a01 + a12);
+    D[2] = fma_(d[2], d[2], a02 + a12);
+    // (01): Q00 Q01 + Q01 Q11 + Q02 Q21,  Q21 = conj Q12
+    Xr[0] = fma_(d[0] + d[1], xr[0], fma_(xr[1], xr[2], xi[1] * xi[2]));
+    Xi[0] = fma_(d[0] + d[1], xi[0], fma_(xi[1], xr[2], -xr[1] * xi[2]));
+    // (02): Q00 Q02 + Q01 Q12 + Q02 Q22
+    Xr[1] = fma_(d[0] + d[2], xr[1], fma_(xr[0], xr[2], -xi[0] * xi[2]));
+    Xi[1] = fma_(d[0] + d[2], xi[1], fma_(xr[0], xi[2], xi[0] * xr[2]));
+    // (12): Q10 Q02 + Q11 Q12 + Q12 Q22,  Q10 = conj Q01
+    Xr[2] = fma_(d[1] + d[2], xr[2], fma_(xr[0], xr[1], xi[0] * xi[1]));
+    Xi[2] = fma_(d[1] + d[2], xi[2], fma_(xr[0], xi[1], -xi[0] * xr[1]));
     const T c1 = T(0.5) * n2;
-    // c0 = (1/3) Re tr(Q Q2) = (1/3) sum_ij Re(Q_ij Q2_ji)
-    T c0 = T(0);
+    // c0 = det Q = (1/3) tr(Q Q2) = (1/3) [sum_i Q_ii Q2_ii + 2 sum_{i<j} Re(Q_ij conj Q2_ij)]
+    T c0 = T(0), c0o = T(0);
 #pragma unroll
-    for (int i = 0; i < 3; i++)
+    for (int i = 0; i < 3; i++) c0 = fma_(d[i], D[i], c0);
 #pragma unroll
-        for (int j = 0; j < 3; j++) {
-            c0 = fma_(Q.re[3 * i + j], Q2.re[3 * j + i], c0);
-            c0 = fma_(-Q.im[3 * i + j], Q2.im[3 * j + i], c0);
-        }
-    c0 *= T(1.0 / 3.0);
-    // series
-    T ar = T(1), ai = T(0), br = T(0), bi = T(0), cr = T(0), ci = T(0);
+    for (int p = 0; p < 3; p++) c0o = fma_(xr[p], Xr[p], fma_(xi[p], Xi[p], c0o));
+    c0 = fma_(T(2), c0o, c0) * T(1.0 / 3.0);
+    // series, two terms per round: odd k adds to the imaginary parts, even k to the real parts; the sign pattern
+    // + - - + of i^k is folded into the recurrence (every even step carries a factor -1)
+    T al = T(1), be = T(0), ga = T(0);
     T f0r = T(1), f0i = T(0), f1r = T(0), f1i = T(0), f2r = T(0), f2i = T(0);
-    // bound on the k-th term: x^k/k! with x = ||Q||_F <= 1
-    T x = sqrt(n2), bound = T(1);
-    for (int k = 1; k <= ExpTerms<T>::max_terms; k++) {
-        const T inv = (T)c_inv_k[k];  // 1/k from a table: an fp64 division is a dozen instructions
-        // (a,b,c) <- (i/k) (c0 c, a + c1 c, b);  i (x + i y) = -y + i x
-        const T tar = c0 * cr, tai = c0 * ci;
-        const T tbr = fma_(c1, cr, ar), tbi = fma_(c1, ci, ai);
-        const T tcr = br, tci = bi;
-        ar = -tai * inv; ai = tar * inv;
-        br = -tbi * inv; bi = tbr * inv;
-        cr = -tci * inv; ci = tcr * inv;
-        f0r += ar; f0i += ai;
-        f1r += br; f1i += bi;
-        f2r += cr; f2i += ci;
-        bound *= x * inv;
+    T bound = T(1);  // x^k / k!, x = ||Q||_F <= 1
+    for (int k = 1; k <= ExpTerms<T>::max_terms; k += 2) {
+        const T inv1 = (T)c_inv_k[k], inv2 = (T)c_inv_k[k + 1];  // 1/k from a table: an fp64 division is a dozen instructions
+        T na = c0 * ga * inv1, nb = fma_(c1, ga, al) * inv1, nc = be * inv1;
+        f0i += na;
+        f1i += nb;
+        f2i += nc;
+        al = -c0 * nc * inv2;
+        be = -fma_(c1, nc, na) * inv2;
+        ga = -nb * inv2;
+        f0r += al;
+        f1r += be;
+        f2r += ga;
+        bound *= n2 * inv1 * inv2;
         if (bound < ExpTerms<T>::tol) break;
     }
     // E = f0 + f1 Q + f2 Q2
+    const int rows = nsq > 0 ? 3 : ROWS;  // squaring needs the whole matrix
 #pragma unroll
-    for (int e = 0; e < 9; e++) {
-        T er = fma_(f1r, Q.re[e], fma_(-f1i, Q.im[e], fma_(f2r, Q2.re[e], -f2i * Q2.im[e])));
-        T ei = fma_(f1r, Q.im[e], fma_(f1i, Q.re[e], fma_(f2r, Q2.im[e], f2i * Q2.re[e])));
-        if (e == 0 || e == 4 || e == 8) {
-            er += f0r;
-            ei += f0i;
+    for (int i = 0; i < 3; i++) {
+        if (i < rows) {
+            E.re[4 * i] = fma_(f1r, d[i], fma_(f2r, D[i], f0r));
+            E.im[4 * i] = fma_(f1i, d[i], fma_(f2i, D[i], f0i));
         }
-        E.re[e] = er;
-        E.im[e] = ei;
+    }
+#pragma unroll
+    for (int p = 0; p < 3; p++) {
+        const int i = I[p], j = J[p];
+        // (i,j): Q_ij = xr + i xi
+        E.re[3 * i + j] = fma_(f1r, xr[p], fma_(-f1i, xi[p], fma_(f2r, Xr[p], -f2i * Xi[p])));
+        E.im[3 * i + j] = fma_(f1r, xi[p], fma_(f1i, xr[p], fma_(f2r, Xi[p], f2i * Xr[p])));
+        // (j,i): Q_ji = xr - i xi
+        if (j < rows) {
+            E.re[3 * j + i] = fma_(f1r, xr[p], fma_(f1i, xi[p], fma_(f2r, Xr[p], f2i * Xi[p])));
+            E.im[3 * j + i] = fma_(-f1r, xi[p], fma_(f1i, xr[p], fma_(-f2r, Xi[p], f2i * Xr[p])));
+        }
     }
     for (int k = 0; k < nsq; k++) {
         M3<T> S;
         mul<false, false, false>(S, E, E);
         E = S;
     }
+}
+
+template <typename T>
+__device__ __forceinline__ void expi_herm(M3<T> &E, const M3<T> &Q) {
+    expi_herm_scaled<3>(E, Q, T(1));
 }
 
 // Q = sum_a q_a T_a (O2), T_a = Gell-Mann / 2

@@ -22,14 +22,13 @@ __global__ void __launch_bounds__(256) link_update_kernel(const int V, const int
         M3<T> Q, Ul, E;
         load_link(Q, P, V, mu, cb);
         load_link_rw(Ul, U, V, mu, cb);
-#pragma unroll
-        for (int e = 0; e < 9; e++) {
-            Q.re[e] *= eps;
-            Q.im[e] *= eps;
+        if (MODE == 1) {
+            expi_herm_scaled<2>(E, Q, eps);
+            mul_top2(R, E, Ul);  // reunit rebuilds row 2
+        } else {
+            expi_herm_scaled<3>(E, Q, eps);
+            mul<false, false, false>(R, E, Ul);
         }
-        expi_herm(E, Q);
-        if (MODE == 1) mul_top2(R, E, Ul);  // reunit rebuilds row 2
-        else mul<false, false, false>(R, E, Ul);
     }
     if (MODE >= 1) reunit(R);
     store_link(R, U, V, mu, cb);

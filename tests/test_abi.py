@@ -114,9 +114,9 @@ def test_tuning_database_roundtrip_and_validation():
     qcd.qcd_tune_clear()
     lat, other = qcd.Lattice((8, 8, 8, 16)), qcd.Lattice((8, 8, 8, 4))
     assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) is None
-    qcd.qcd_tune_set(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index("site256"), (8, 4, 4, 2))
+    qcd.qcd_tune_set(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index("plane"), (8, 4, 2, 2))
     qcd.qcd_tune_set(lat, qcd.F64, qcd.EVEN, qcd.KERNEL_LINK_UPDATE, threads=64)
-    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) == (1, (8, 4, 4, 2), 0)
+    assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) == (1, (8, 4, 2, 2), 0)
     assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ODD, qcd.KERNEL_LINK_UPDATE) == (0, (0, 0, 0, 0), 64)  # EVEN/ODD share
     assert qcd.qcd_tune_get(lat, qcd.F32, qcd.ALL, qcd.KERNEL_FORCE) is None  # keyed on precision
     assert qcd.qcd_tune_get(other, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) is None  # and on the extents
@@ -124,6 +124,7 @@ def test_tuning_database_roundtrip_and_validation():
     assert qcd.qcd_tune_get(lat, qcd.F64, qcd.ALL, qcd.KERNEL_FORCE) == (0, (0, 0, 0, 0), 0)
     for bad in [dict(kernel=qcd.KERNEL_FORCE, variant=9), dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(3, 2, 2, 2)),
                 dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(8, 8, 8, 2)),  # 1024 sites > 128-thread block
+                dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(8, 4, 4, 4)),  # 512 sites = 256 per parity > 128
                 dict(kernel=qcd.KERNEL_FORCE, variant=0, tile=(5, 2, 2, 2)), dict(kernel=qcd.KERNEL_MOM_UPDATE, threads=48),
                 dict(kernel=qcd.KERNEL_LINK_UPDATE, threads=512), dict(kernel=7, threads=64)]:
         with pytest.raises(qcd.QcdError) as e:

@@ -284,26 +284,16 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("variant,tile", [("site", None), ("site", "4,2,2,2"), ("site+rec", None), ("site256", None),
-                                          ("site256", "4,2,2,2"), ("pipe", None), ("pipe", "4,2,2,2"),
-                                          ("plane", None), ("plane", "4,2,2,2"), ("link", None), ("tile", None),
-                                          ("tile", "8,2,2,4"), ("tile", "4,4,4,4"), ("plaq", None),
-                                          ("plaq", "8,4,2,2"), ("plaq", "4,2,4,2")])
+@pytest.mark.parametrize("variant,tile", [("plane", None), ("plane", (4, 2, 2, 2)), ("plane", (8, 4, 2, 2)),
+                                          ("plane", (4, 4, 4, 2)), ("plane", (2, 2, 2, 2)), ("staple", None),
+                                          ("staple", (4, 2, 2, 2)), ("staple", (8, 2, 2, 4))])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 4), (16, 8, 8, 16)])
-def test_force_kernel_variants(qcd, orc_omp, monkeypatch, prec, variant, tile, dims):
-    """every selectable force kernel (QCD_FORCE_VARIANT, QCD_TILE: the block-shape sweep knobs) against the
-    oracle, fused and unfused, on SU(3) links (the plaq variant needs unitary links), over several tiles
-    and with tiles that span a whole extent (periodic wrap inside the tile)"""
-    if variant.endswith("+rec"):  # two-row loads of SU(3) links (third row rebuilt in registers)
-        variant = variant[:-4]
-        monkeypatch.setenv("QCD_SU3_REC", "1")
-    monkeypatch.setenv("QCD_FORCE_VARIANT", variant)
-    if tile:
-        if any(d % t for d, t in zip(dims, map(int, tile.split(",")))):
-            pytest.skip("tile does not divide the lattice")
-        monkeypatch.setenv("QCD_TILE", tile)
-    else:
-        monkeypatch.delenv("QCD_TILE", raising=False)
+def test_force_kernel_variants(qcd, orc_omp, prec, variant, tile, dims):
+    """both force kernels (the tuner's database is the knob: variant and 4-D block tile) against the oracle,
+    fused and unfused, over several tiles, with tiles that span a whole extent (periodic wrap inside the
+    tile) and with blocks that are not a whole number of warps"""
+    if tile and any(d % t for d, t in zip(dims, tile)):
+        pytest.skip("tile does not divide the lattice")
     lat = qcd.Lattice(dims)
     beta, eps = 6.0, 0.07
     U = round_to(prec, orc_omp.hot_start(dims, inputs.config_seed(2), 0.5))
@@ -311,11 +301,23 @@ def test_force_kernel_variants(qcd, orc_omp, monkeypatch, prec, variant, tile, d
     Fr = orc_omp.gauge_force(dims, beta, U)
     dU = dev(qcd, lat, U, prec)
     F = lat.new_matrix_field(tdtype(prec))
-    qcd.qcd_gauge_force(lat, dU, F, beta)
-    assert rel(host(qcd, lat, F), Fr) < TOL[prec]
-    dP = dev(qcd, lat, P, prec)
-    qcd.qcd_force_mom_update(lat, dU, dP, beta, eps)
-    assert rel(host(qcd, lat, dP), P + eps * Fr) < TOL[prec]
+    p = qcd.F64 if prec == "f64" else qcd.F32
+    try:
+        for subset in (qcd.ALL, qcd.EVEN):
+            qcd.qcd_tune_set(lat, p, subset, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index(variant), tile)
+        qcd.qcd_gauge_force(lat, dU, F, beta)
+        assert rel(host(qcd, lat, F), Fr) < TOL[prec]
+        dP = dev(qcd, lat, P, prec)
+        qcd.qcd_force_mom_update(lat, dU, dP, beta, eps)
+        assert rel(host(qcd, lat, dP), P + eps * Fr) < TOL[prec]
+        par = orc_omp.map(dims, O.MAP_PARITY)
+        dP = dev(qcd, lat, P, prec)
+        qcd.qcd_force_mom_update(lat, dU, dP, beta, eps, subset=qcd.ODD)
+        want = P.copy()
+        want[par == 1] += eps * Fr[par == 1]
+        assert rel(host(qcd, lat, dP), want) < TOL[prec]
+    finally:
+        qcd.qcd_tune_clear()
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
