@@ -236,9 +236,9 @@ def run_ours(args, cfg):
     work = torch.empty(lat.md_host_work_bytes(qcd.F64 if args.dtype == "f64" else qcd.F32) // rbytes, dtype=dtype,
                        device="cuda")
     tmp = work[: V * 72]
-    qcd.qcd_unpack(lat, 72, U, tmp)
+    qcd.qcd_unpack(lat, 72, qcd.LAYOUT_PAIRS, U, tmp)
     hU.copy_(tmp)
-    qcd.qcd_unpack(lat, 72, P, tmp)
+    qcd.qcd_unpack(lat, 72, qcd.LAYOUT_PAIRS, P, tmp)
     hP.copy_(tmp)
     qcd.qcd_md_host(lat, hU, hP, beta, eps, 1, work)  # warm-up
     barrier()

@@ -42,13 +42,16 @@
  *   doubles.  qcd_lattice is host-only, immutable after creation and may be shared across threads.
  *
  * ERRORS
- *   Return code only: no exceptions, no abort, no printing.  On a nonzero return nothing was
- *   enqueued.  qcd_last_error() returns a thread-local text for the last nonzero return.
+ *   Return code only: no exceptions, no abort, no printing.  Arguments are validated before the first
+ *   launch, so on any return other than QCD_ECUDA nothing was enqueued; QCD_ECUDA (a launch the CUDA runtime
+ *   refused) can leave the earlier kernels of a multi-launch call (qcd_md_step, qcd_leapfrog*, qcd_trajectory,
+ *   qcd_nested_leapfrog, qcd_md_host) on the stream.  qcd_last_error() returns a thread-local text for the
+ *   last nonzero return.
  *     QCD_EINVAL      NULL pointer, unknown enum value, nsub < 1, ncomp < 1 ...
  *     QCD_EDIMS       an extent is odd or < 2, or 36 V >= 2^32
  *     QCD_EALIGN      a field pointer is not 16-byte aligned
  *     QCD_EALIAS      input and output overlap where the operation forbids it
- *     QCD_EWORKSPACE  reserved (workspace too small cannot be detected from a raw pointer)
+ *     QCD_EWORKSPACE  the workspace is too small (calls that take its size, and tuned tiles with too many blocks)
  *     QCD_ECUDA       the CUDA runtime reported a launch error (text in qcd_last_error)
  *   Scalars beta, eps, sigma are double and rounded to float once for QCD_F32.
  */
@@ -67,6 +70,7 @@ typedef struct qcd_lattice qcd_lattice; /* opaque, host side */
 enum { QCD_F32 = 0, QCD_F64 = 1 };
 enum { QCD_ALL = 0, QCD_EVEN = 1, QCD_ODD = 2 };
 enum { QCD_SUM_SCALAR = 0, QCD_SUM_NORM2 = 1, QCD_SUM_RETR = 2 };
+enum { QCD_LAYOUT_REAL = 0, QCD_LAYOUT_PAIRS = 1 }; /* device layout of a field: NC = ncomp reals, or ncomp/2 pairs */
 enum { QCD_OK = 0, QCD_EINVAL = 1, QCD_EDIMS = 2, QCD_EALIGN = 3, QCD_EALIAS = 4, QCD_EWORKSPACE = 5,
        QCD_ECUDA = 6 };
 /* qcd_get_map `which`: maps are indexed by the lexicographic index and hold lexicographic indices,
@@ -142,8 +146,8 @@ int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_a
                   void *workspace, void *stream);
 
 /* Global / subset sum [O12] ("sum") of a per-site quantity of `field`:
- *   QCD_SUM_SCALAR  real field with ncomp components: out[c] = sum_x field_c(x), c < ncomp <= 64
- *   QCD_SUM_NORM2   field with ncomp reals per site (ncomp even): out[0] = sum_x sum_i field_i(x)^2
+ *   QCD_SUM_SCALAR  real field (QCD_LAYOUT_REAL) with ncomp components: out[c] = sum_x field_c(x), c < ncomp <= 64
+ *   QCD_SUM_NORM2   pair-layout field (QCD_LAYOUT_PAIRS) with ncomp reals per site: out[0] = sum_x sum_i field_i(x)^2
  *                   (ncomp = 72 on P gives the kinetic energy sum tr P^2)
  *   QCD_SUM_RETR    matrix field of ncomp/18 matrices per site: out[0] = sum_x sum_m Re tr M_m(x)
  * Deterministic two-pass reduction in double.  out: device doubles. */
@@ -167,8 +171,8 @@ int qcd_md_step(const qcd_lattice *lat, int prec, double beta, double eps_p, dou
  * out_avg: sum_{x,mu} Re tr W_mu(x) = 4 sum_{x,mu<nu} Re tr P_mu_nu(x)), out[1] = K = sum |P_ij|^2 of the
  * UPDATED momenta (as qcd_sum NORM2).  Saves the two extra passes (1152 B/site) per observed step.  Device
  * doubles; workspace as qcd_workspace_bytes.  Deterministic run to run at a fixed block shape (one partial
- * per block, fixed order); not per timeslice.  QCD_EWORKSPACE if the lattice's workspace cannot hold
- * two doubles per block. */
+ * per block, fixed order); per timeslice: see qcd_trajectory.  QCD_EWORKSPACE if the lattice's workspace cannot
+ * hold two doubles per block. */
 int qcd_force_mom_update_sums(const qcd_lattice *lat, int prec, double beta, double eps, const void *U, void *P,
                               double *out, void *workspace, void *stream);
 /* qcd_leapfrog whose last momentum update is qcd_force_mom_update_sums: out[0] = plaquette average and
@@ -189,6 +193,23 @@ int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, doubl
  * The final links are always left in U (an odd nsteps starts with one two-kernel in-place step). */
 int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U,
                              void *P, void *U_work, void *stream);
+
+/* Leapfrog trajectory [O11] that also returns the observables of every step (BASELINE.json configs 4, 5: "per-step
+ * reunitarization and reductions ... sumMulti of plaquette per timeslice ... kinetic-energy sum"; PAPER.md:26 sum /
+ * sumMulti, fused into the site loop as in PAPER.md:32).  Built from single-pass steps like
+ * qcd_leapfrog_single_pass; the plaquette sums and the kinetic energy are by-products of the force kernel, so a step
+ * costs no extra pass over the fields.  Same U, P as qcd_leapfrog up to rounding order.
+ *   obs    device double[2*(nsteps+1)]:  obs[2k] = plaquette average of U_k (U after k link updates), k = 0..nsteps;
+ *          obs[1] = K of the initial momenta, obs[2k+1] (0 < k < nsteps) = K of the momenta after the full kick that
+ *          follows link update k (time (k+1/2) eps), obs[2 nsteps + 1] = K of the final momenta.  Hence
+ *          H_start = obs[1] + beta 6V (1 - obs[0]),  H_end = obs[2n+1] + beta 6V (1 - obs[2n]),  dH = H_end - H_start.
+ *   per_t  device double[(nsteps+1)*Lt] or NULL: plaquette average of every timeslice of U_k (R13), row k.
+ *   U_work scratch gauge field, qcd_field_bytes(lat, prec, 72) bytes; the final links are always left in U.
+ *   workspace, workspace_bytes: at least qcd_workspace_bytes(lat), else QCD_EWORKSPACE (also returned when a tuned
+ *          tile has more blocks than the workspace has room for).  All checks are made before anything is enqueued.
+ * Deterministic run to run at a fixed launch configuration (one partial per block, fixed order). */
+int qcd_trajectory(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
+                   void *U_work, double *obs, double *per_t, void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- anisotropic Wilson action and multi-timescale integrator ------------------
  * The paper's demonstration ran an anisotropic Wilson gauge action with multi-timescale
@@ -220,8 +241,7 @@ int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2]
  * PAPER.md:83): Gaussian fill of a spin-colour vector field and its norm / inner-product reductions
  * (PAPER.md:26).  A spin-colour vector has 12 complex components per site, k = 3*spin + colour; device
  * layout: complex pairs, NC = 12 units per site, component k of site cb at unit index ((cb>>5)*12 + k)*32 + (cb&31) (24 reals per site;
- * qcd_pack / qcd_unpack use this pair layout whenever ncomp is a multiple of 18 or of 24; canonical
- * layout [s][k][re,im]).  [O15] eta_k(x) = (g0 + i g1)/sqrt(2), (g0,g1) the Box-Muller pair of generator
+ * qcd_pack / qcd_unpack with QCD_LAYOUT_PAIRS; canonical layout [s][k][re,im]).  [O15] eta_k(x) = (g0 + i g1)/sqrt(2), (g0,g1) the Box-Muller pair of generator
  * block (lexicographic site, 64 + k, stream_id, purpose 4): <|eta_k|^2> = 1, weight exp(-eta^dag eta).
  * Writes only the subset's sites.  The norm is qcd_sum(QCD_SUM_NORM2, ncomp = 24). */
 int qcd_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id,
@@ -266,10 +286,14 @@ int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int 
 /* ---- helpers (not on the hot path) -------------------------------------------------------- */
 
 /* canonical lexicographic AoS (device, exactly V*ncomp reals) -> device layout (qcd_field_bytes bytes), and back.
- * ncomp reals per site; ncomp a multiple of 18 or 24 selects the pair layout (NC = ncomp/2), any other ncomp
- * the real layout (NC = ncomp).  For matrix fields ncomp = 72.  Input and output must not overlap. */
-int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream);
-int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa, void *lex_aos, void *stream);
+ * ncomp reals per site; `layout` says which device layout the field has: QCD_LAYOUT_PAIRS (NC = ncomp/2 (re,im)
+ * units per site, ncomp even: matrix fields with ncomp = 72, spin-colour vectors with ncomp = 24, what
+ * QCD_SUM_NORM2 / QCD_SUM_RETR / qcd_inner_product read) or QCD_LAYOUT_REAL (NC = ncomp reals per site, what
+ * QCD_SUM_SCALAR reads).  Input and output must not overlap.  QCD_EDIMS if NC (V + 32) >= 2^32. */
+int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, int layout, const void *lex_aos, void *dev_soa,
+             void *stream);
+int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, int layout, const void *dev_soa, void *lex_aos,
+               void *stream);
 /* index / subset maps [O1] into dev_out (int32[V]) */
 int qcd_get_map(const qcd_lattice *lat, int which, int32_t *dev_out, void *stream);
 /* hot start [O5]: U_mu(x) = exp(i sigma Q), Q = sum q_a T_a, q_a ~ N(0,1) from purpose 0 */

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libqcdmd.so")
 F32, F64 = 0, 1
 ALL, EVEN, ODD = 0, 1, 2
 SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
+LAYOUT_REAL, LAYOUT_PAIRS = 0, 1
 OK, EINVAL, EDIMS, EALIGN, EALIAS, EWORKSPACE, ECUDA = range(7)
 KERNEL_FORCE, KERNEL_LINK_UPDATE, KERNEL_MOM_UPDATE = 0, 1, 2
 FORCE_VARIANTS = ("staple", "plane")  # index = QCD_FORCE_* value
@@ -46,6 +47,7 @@ SIGNATURES = {
     "qcd_leapfrog_energy": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp, _vp]),
     "qcd_md_step_single_pass": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "qcd_leapfrog_single_pass": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
+    "qcd_trajectory": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "qcd_gauge_force_aniso": (_i, [_vp, _i, _i, _d, _d, _vp, _vp, _vp]),
     "qcd_force_mom_update_aniso": (_i, [_vp, _i, _i, _d, _d, _d, _vp, _vp, _vp]),
     "qcd_plaquette_st": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
@@ -57,8 +59,8 @@ SIGNATURES = {
     "qcd_tune_set": (_i, [_vp, _i, _i, _i, _i, C.POINTER(C.c_int * 4), _i]),
     "qcd_tune_get": (_i, [_vp, _i, _i, _i, C.POINTER(_i), C.POINTER(C.c_int * 4), C.POINTER(_i)]),
     "qcd_tune_clear": (_i, []),
-    "qcd_pack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
-    "qcd_unpack": (_i, [_vp, _i, _i, _vp, _vp, _vp]),
+    "qcd_pack": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp]),
+    "qcd_unpack": (_i, [_vp, _i, _i, _i, _vp, _vp, _vp]),
     "qcd_get_map": (_i, [_vp, _i, _vp, _vp]),
     "qcd_hot_start": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
     "qcd_perturb": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
@@ -155,7 +157,7 @@ class Lattice:
         return torch.zeros((self.nchunks, 12, 32, 2), dtype=dtype, device=device)
 
     def new_pair_field(self, nc, dtype=torch.float64, device="cuda"):
-        """[chunk][nc][32][2]: nc complex units per site (2*nc a multiple of 18 or 24 for qcd_pack)"""
+        """[chunk][nc][32][2]: nc complex units per site (QCD_LAYOUT_PAIRS)"""
         return torch.zeros((self.nchunks, nc, 32, 2), dtype=dtype, device=device)
 
     def new_real_field(self, ncomp, dtype=torch.float64, device="cuda"):
@@ -241,6 +243,12 @@ def qcd_leapfrog_single_pass(lat, U, P, U_work, beta, eps, nsteps, stream=None):
                                         _stream(stream)))
 
 
+def qcd_trajectory(lat, U, P, U_work, beta, eps, nsteps, obs, per_t, workspace, stream=None):
+    _check(lib.qcd_trajectory(lat.handle, _prec(U), beta, eps, nsteps, _ptr(U), _ptr(P), _ptr(U_work), _ptr(obs),
+                              _ptr(per_t), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                              _stream(stream)))
+
+
 def qcd_gauge_force_aniso(lat, U, F, beta_s, beta_t, subset=ALL, stream=None):
     _check(lib.qcd_gauge_force_aniso(lat.handle, _prec(U), subset, beta_s, beta_t, _ptr(U), _ptr(F), _stream(stream)))
 
@@ -292,12 +300,12 @@ def qcd_tune_clear():
     _check(lib.qcd_tune_clear())
 
 
-def qcd_pack(lat, ncomp, lex_aos, dev_soa, stream=None):
-    _check(lib.qcd_pack(lat.handle, _prec(dev_soa), ncomp, _ptr(lex_aos), _ptr(dev_soa), _stream(stream)))
+def qcd_pack(lat, ncomp, layout, lex_aos, dev_soa, stream=None):
+    _check(lib.qcd_pack(lat.handle, _prec(dev_soa), ncomp, layout, _ptr(lex_aos), _ptr(dev_soa), _stream(stream)))
 
 
-def qcd_unpack(lat, ncomp, dev_soa, lex_aos, stream=None):
-    _check(lib.qcd_unpack(lat.handle, _prec(dev_soa), ncomp, _ptr(dev_soa), _ptr(lex_aos), _stream(stream)))
+def qcd_unpack(lat, ncomp, layout, dev_soa, lex_aos, stream=None):
+    _check(lib.qcd_unpack(lat.handle, _prec(dev_soa), ncomp, layout, _ptr(dev_soa), _ptr(lex_aos), _stream(stream)))
 
 
 def qcd_get_map(lat, which, out, stream=None):
@@ -329,7 +337,7 @@ def field_to_device(lat, host_array, dtype=torch.float64):
     """numpy complex128 [V,4,3,3] (canonical layout) -> device matrix field of `dtype`"""
     t = torch.view_as_real(torch.from_numpy(host_array)).reshape(-1).to(dtype).cuda()
     out = lat.new_matrix_field(dtype)
-    qcd_pack(lat, 72, t, out)
+    qcd_pack(lat, 72, LAYOUT_PAIRS, t, out)
     torch.cuda.current_stream().synchronize()
     return out
 
@@ -337,5 +345,5 @@ def field_to_device(lat, host_array, dtype=torch.float64):
 def field_to_host(lat, dev_field):
     """device matrix field -> numpy complex128 [V,4,3,3]"""
     t = torch.empty(lat.V * 72, dtype=dev_field.dtype, device=dev_field.device)  # canonical: no padding
-    qcd_unpack(lat, 72, dev_field, t)
+    qcd_unpack(lat, 72, LAYOUT_PAIRS, dev_field, t)
     return t.to(torch.float64).cpu().numpy().view("complex128").reshape(lat.V, 4, 3, 3)

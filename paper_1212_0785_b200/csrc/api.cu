@@ -55,6 +55,11 @@ static int check_alias2(const void *a, size_t bytes_a, const void *b, size_t byt
 static int check_alias(const void *a, const void *b, size_t bytes, const char *fn) {
     return check_alias2(a, bytes, b, bytes, fn);
 }
+// the kernels index the units of a field with 32 bits: nc units per site need nc (V + 32) < 2^32
+static int check_units(const qcd_lattice *lat, long long nc, const char *fn) {
+    if (nc * ((long long)lat->p.V + 32) >= (1ll << 32)) return bad(QCD_EDIMS, "%s: units per site x V must be < 2^32", fn);
+    return QCD_OK;
+}
 
 }  // namespace qcd
 
@@ -205,6 +210,7 @@ int qcd_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, c
     QCD_TRY(check_common(lat, prec, fn));
     QCD_TRY(check_subset(subset, fn));
     QCD_TRY(check_sum_args(kind, ncomp, fn));
+    QCD_TRY(check_units(lat, kind == QCD_SUM_SCALAR ? ncomp : ncomp / 2, fn));
     QCD_TRY(check_ptr(field, fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
     return launch_sum(lat, prec, subset, kind, ncomp, field, out, (double *)workspace, (cudaStream_t)stream);
@@ -215,6 +221,7 @@ int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const v
     const char *fn = "qcd_sum_multi";
     QCD_TRY(check_common(lat, prec, fn));
     QCD_TRY(check_sum_args(kind, ncomp, fn));
+    QCD_TRY(check_units(lat, kind == QCD_SUM_SCALAR ? ncomp : ncomp / 2, fn));
     QCD_TRY(check_ptr(field, fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
     if (nsub < 1 || nsub > MAX_NSUB) return bad(QCD_EINVAL, "%s: nsub out of range [1,4096]", fn);
@@ -261,7 +268,8 @@ int qcd_force_mom_update_sums(const qcd_lattice *lat, int prec, double beta, dou
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
-    return launch_force_sums(lat, prec, beta, eps, 0.0, U, P, nullptr, out, (double *)workspace, (cudaStream_t)stream);
+    return launch_force_sums(lat, prec, beta, eps, 0.0, U, P, nullptr, out, out + 1, nullptr, (double *)workspace,
+                             (cudaStream_t)stream);
 }
 
 int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
@@ -279,7 +287,7 @@ int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double ep
         QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
         if (k < nsteps - 1) QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps, U, P, true, st));
     }
-    return launch_force_sums(lat, prec, beta, 0.5 * eps, 0.0, U, P, nullptr, out, (double *)workspace, st);
+    return launch_force_sums(lat, prec, beta, 0.5 * eps, 0.0, U, P, nullptr, out, out + 1, nullptr, (double *)workspace, st);
 }
 
 int qcd_md_step_single_pass(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
@@ -324,6 +332,56 @@ int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, doub
         other = t;
     }
     return launch_gauge_force(lat, prec, QCD_ALL, beta, 0.5 * eps, cur, P, true, st);
+}
+
+int qcd_trajectory(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P, void *U_work,
+                   double *obs, double *per_t, void *workspace, size_t workspace_bytes, void *stream) {
+    const char *fn = "qcd_trajectory";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U_work, fn));
+    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    QCD_TRY(check_alias(U, P, fb, fn));
+    QCD_TRY(check_alias(U, U_work, fb, fn));
+    QCD_TRY(check_alias(P, U_work, fb, fn));
+    if (nsteps < 1) return bad(QCD_EINVAL, "%s: nsteps < 1", fn);
+    if (!obs || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
+    if (workspace_bytes < qcd_workspace_bytes(lat)) return bad(QCD_EWORKSPACE, "%s: workspace smaller than qcd_workspace_bytes", fn);
+    QCD_TRY(force_sums_check(lat, prec));
+    cudaStream_t st = (cudaStream_t)stream;
+    double *ws = (double *)workspace;
+    double *scratch = ws + lat->workspace_doubles - 8;  // K after the opening half kick has no slot in obs
+    const int Lt = lat->p.L[3];
+    // One kick (+ link update into `to` when to != NULL) with plaq(U), per-timeslice plaq(U) and K(P after) as
+    // by-products; the per-timeslice values fall back to the stand-alone plaquette kernel when the launch
+    // configuration cannot give them.
+    auto kick = [&](double eps_p, void *from, void *to, double *o_plaq, double *o_K, double *o_per_t) -> int {
+        int rc = launch_force_sums(lat, prec, beta, eps_p, eps, from, P, to, o_plaq, o_K, o_per_t, ws, st);
+        if (rc == -1) {
+            QCD_TRY(launch_plaquette(lat, prec, from, o_plaq, o_per_t, ws, st));
+            rc = launch_force_sums(lat, prec, beta, eps_p, eps, from, P, to, o_plaq, o_K, nullptr, ws, st);
+        }
+        return rc;
+    };
+    // O11 regrouped as in qcd_leapfrog_single_pass; step k reports plaq(U_k) and K of the momenta after its kick
+    QCD_TRY(launch_sum(lat, prec, QCD_ALL, QCD_SUM_NORM2, 72, P, obs + 1, ws, st));  // K of the initial momenta
+    void *cur = U, *other = U_work;
+    int k = 0;
+    if (nsteps & 1) {  // keep the number of ping-pong steps even so the result lands in U
+        QCD_TRY(kick(0.5 * eps, U, nullptr, obs, scratch, per_t));
+        QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
+        k = 1;
+    }
+    for (; k < nsteps; k++) {
+        QCD_TRY(kick(k == 0 ? 0.5 * eps : eps, cur, other, obs + 2 * k, k == 0 ? scratch : obs + 2 * k + 1,
+                     per_t ? per_t + (size_t)k * Lt : nullptr));
+        void *t = cur;
+        cur = other;
+        other = t;
+    }
+    return kick(0.5 * eps, cur, nullptr, obs + 2 * nsteps, obs + 2 * nsteps + 1,
+                per_t ? per_t + (size_t)nsteps * Lt : nullptr);
 }
 
 int qcd_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t, const void *U,
@@ -401,6 +459,7 @@ static int check_inner(const qcd_lattice *lat, int prec, int nc, const void *a, 
     QCD_TRY(check_ptr(a, fn));
     QCD_TRY(check_ptr(b, fn));
     if (nc < 1) return bad(QCD_EINVAL, "%s: nc < 1", fn);
+    QCD_TRY(check_units(lat, nc, fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
     return QCD_OK;
 }
@@ -468,25 +527,32 @@ int qcd_tune_clear(void) {
     return QCD_OK;
 }
 
-int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex_aos, void *dev_soa, void *stream) {
+static int check_layout(const qcd_lattice *lat, int ncomp, int layout, const char *fn) {
+    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    if (layout != QCD_LAYOUT_REAL && layout != QCD_LAYOUT_PAIRS) return bad(QCD_EINVAL, "%s: unknown layout", fn);
+    if (layout == QCD_LAYOUT_PAIRS && (ncomp & 1)) return bad(QCD_EINVAL, "%s: the pair layout needs an even ncomp", fn);
+    return check_units(lat, layout == QCD_LAYOUT_PAIRS ? ncomp / 2 : ncomp, fn);
+}
+
+int qcd_pack(const qcd_lattice *lat, int prec, int ncomp, int layout, const void *lex_aos, void *dev_soa, void *stream) {
     const char *fn = "qcd_pack";
     QCD_TRY(check_common(lat, prec, fn));
-    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    QCD_TRY(check_layout(lat, ncomp, layout, fn));
     QCD_TRY(check_ptr(lex_aos, fn));
     QCD_TRY(check_ptr(dev_soa, fn));
     // the canonical array has exactly V sites, the device field whole chunks of 32
     QCD_TRY(check_alias2(lex_aos, (size_t)lat->p.V * ncomp * real_bytes(prec), dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
-    return launch_pack(lat, prec, ncomp, lex_aos, dev_soa, false, (cudaStream_t)stream);
+    return launch_pack(lat, prec, ncomp, layout == QCD_LAYOUT_PAIRS, lex_aos, dev_soa, false, (cudaStream_t)stream);
 }
 
-int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, const void *dev_soa, void *lex_aos, void *stream) {
+int qcd_unpack(const qcd_lattice *lat, int prec, int ncomp, int layout, const void *dev_soa, void *lex_aos, void *stream) {
     const char *fn = "qcd_unpack";
     QCD_TRY(check_common(lat, prec, fn));
-    if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);
+    QCD_TRY(check_layout(lat, ncomp, layout, fn));
     QCD_TRY(check_ptr(lex_aos, fn));
     QCD_TRY(check_ptr(dev_soa, fn));
     QCD_TRY(check_alias2(lex_aos, (size_t)lat->p.V * ncomp * real_bytes(prec), dev_soa, qcd_field_bytes(lat, prec, ncomp), fn));
-    return launch_pack(lat, prec, ncomp, dev_soa, lex_aos, true, (cudaStream_t)stream);
+    return launch_pack(lat, prec, ncomp, layout == QCD_LAYOUT_PAIRS, dev_soa, lex_aos, true, (cudaStream_t)stream);
 }
 
 int qcd_get_map(const qcd_lattice *lat, int which, int32_t *dev_out, void *stream) {
@@ -535,14 +601,14 @@ int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int n
         set_error("%s: H2D copy: %s", fn, cudaGetErrorString(e));
         return QCD_ECUDA;
     }
-    QCD_TRY(launch_pack(lat, prec, 72, stageU, U, false, st));
-    QCD_TRY(launch_pack(lat, prec, 72, stageP, P, false, st));
+    QCD_TRY(launch_pack(lat, prec, 72, true, stageU, U, false, st));
+    QCD_TRY(launch_pack(lat, prec, 72, true, stageP, P, false, st));
     for (int k = 0; k < nsteps; k++) {
         QCD_TRY(launch_gauge_force(lat, prec, QCD_ALL, beta, eps, U, P, true, st));
         QCD_TRY(launch_link_update(lat, prec, QCD_ALL, eps, P, U, 1, st));
     }
-    QCD_TRY(launch_pack(lat, prec, 72, U, stageU, true, st));
-    QCD_TRY(launch_pack(lat, prec, 72, P, stageP, true, st));
+    QCD_TRY(launch_pack(lat, prec, 72, true, U, stageU, true, st));
+    QCD_TRY(launch_pack(lat, prec, 72, true, P, stageP, true, st));
     e = cudaMemcpyAsync(U_host, stageU, hb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P_host, stageP, hb, cudaMemcpyDeviceToHost, st);
     if (e != cudaSuccess) {

@@ -195,7 +195,7 @@ __device__ __forceinline__ void force_from_ta(M3<T> &F, const TA<T> &a, T c) {
 }
 
 // The pending TA parts, four directions x nine reals per thread.  TMEM = true: in Tensor Memory (tmem.cuh; the
-// block must be exactly four full warps); false: in shared memory, component j of direction d at
+// block must be whole warps, at most four); false: in shared memory, component j of direction d at
 // [(d*9 + j)*FORCE_NT + thread].
 template <typename T, bool TMEM>
 struct Pend {
@@ -243,8 +243,10 @@ struct Pend {
 // "single pass, ping-pong U"): Uout_mu(x) = reunit(exp(i eps_u P_mu(x)) U_mu(x)) is written to a second gauge
 // field (neighbouring threads still read the old U).  ANISO (R19): the staples of plane
 // (mu,nu) carry the weight wt if mu or nu is the time direction, else ws (c is then 1/12); planes of weight zero
-// are skipped.  SUMS (needs FUSED): sum Re tr W_mu(x) = 4 sum_{mu<nu} Re tr P_mu_nu and K = sum |P_ij|^2 of the
-// updated momenta as by-products (PAPER.md:26 fused as in PAPER.md:32), one fp64 partial pair per block.
+// are skipped.  SUMS (needs FUSED): sum_{mu<nu} Re tr P_mu_nu(x) over the block's sites (the closed plaquettes are
+// exactly the six based at x, so a block whose tile lies in one timeslice also yields that timeslice's share,
+// R13) and K = sum |P_ij|^2 of the updated momenta as by-products (PAPER.md:26 fused as in PAPER.md:32), one fp64
+// partial pair per block.
 template <typename T, bool FUSED, bool EARLYP, bool LINK, bool ANISO, bool SUMS, bool TMEM>
 __global__ void __launch_bounds__(FORCE_NT, 3)
     force_plane_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */, const T eps,
@@ -303,7 +305,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
             load_link(X, U, V, mu, cb);
             TA<T> t;
             const T tr = mul_ta<false, SUMS>(t, X, Y);
-            if (SUMS) sumW += 2.0 * (double)tr;  // Re tr Pl = Re tr Pl^dag
+            if (SUMS) sumW += (double)tr;  // Re tr P_mu_nu(x): the six plaquettes based at x, each exactly once
             pend.template add<1>(mu, t);
             pend.template add<-1>(nu, t);
         }
@@ -331,8 +333,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
         load_link(Um, U, V, mu, cb);
         TA<T> acc;
         pend.load(mu, acc);
-        const T tr = mul_ta<true, SUMS>(acc, Um, A);
-        if (SUMS) sumW += (double)tr;
+        mul_ta<true, false>(acc, Um, A);
         force_from_ta(F, acc, c);
         finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
         const int tf = df[0], tb = db[0];
@@ -523,7 +524,7 @@ static void launch_force_k(const qcd_lattice *lat, const ForceSel &fs, T c, T ep
     if (fs.variant == QCD_FORCE_STAPLE)
         force_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS><<<blocks, threads, 0, st>>>(lat->p, tp, c, eps, U, out, eps_u,
                                                                                         Uout, ws, wt, partial);
-    else if (threads == FORCE_NT)  // four full warps: the pending parts live in Tensor Memory
+    else if (threads % 32 == 0)  // whole warps: the pending parts live in Tensor Memory
         force_plane_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS, true><<<blocks, threads, 0, st>>>(
             lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial);
     else
@@ -572,22 +573,32 @@ int launch_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, doubl
                            : launch_force_aniso_t<float>(lat, subset, fs, ws, wt, eps, U, out, fused_mom, st);
 }
 
-// workspace of the kernels that reduce as a by-product: two doubles per block
-int force_sums_blocks(const qcd_lattice *lat, int prec) {
+// the by-product sums need two doubles of workspace per block of the current launch configuration
+int force_sums_check(const qcd_lattice *lat, int prec) {
     const ForceSel fs = force_sel(lat, prec, QCD_ALL);
-    return fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
+    const size_t blocks = (size_t)fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
+    if (2 * blocks + 8 > lat->workspace_doubles) {
+        set_error("force sums: the workspace cannot hold two doubles per block of the tuned tile");
+        return QCD_EWORKSPACE;
+    }
+    return QCD_OK;
 }
 
 // Force + momentum update (+ link update when Uout != NULL) with the plaquette and kinetic-energy sums as
-// by-products (subset ALL).  out[0] = plaquette average of U, out[1] = K of the updated P.
+// by-products (subset ALL).  out_plaq[0] = plaquette average of U, out_K[0] = K of the updated P, out_per_t (or
+// NULL) = plaquette average per timeslice (Lt doubles).  Returns -1 (nothing enqueued) when out_per_t is asked
+// for but the launch configuration cannot give it (staple variant, or a tile that spans several timeslices).
 template <typename T>
 static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, double beta, double eps_p, double eps_u,
-                               const void *U, void *P, void *Uout, double *out, double *ws, cudaStream_t st) {
+                               const void *U, void *P, void *Uout, double *out_plaq, double *out_K, double *out_per_t,
+                               double *ws, cudaStream_t st) {
     const int blocks = fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
     if ((size_t)2 * blocks > lat->workspace_doubles) {
         set_error("force sums: workspace too small");
         return QCD_EWORKSPACE;
     }
+    const bool plane = fs.variant != QCD_FORCE_STAPLE;
+    if (out_per_t && !(plane && fs.tp.T[3] == 1)) return -1;
     const T c = (T)(beta / 12.0);
     if (Uout)
         launch_force_k<T, true, true, false, true>(lat, fs, c, (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u,
@@ -596,15 +607,22 @@ static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, doubl
         launch_force_k<T, true, false, false, true>(lat, fs, c, (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, T(0),
                                                     nullptr, T(0), T(0), ws, st);
     QCD_TRY_RC(check_launch("force sums"));
-    QCD_TRY_RC(launch_sum_partials(ws, blocks, 1.0 / (72.0 * (double)lat->p.V), out, st));
-    return launch_sum_partials(ws + blocks, blocks, 1.0, out + 1, st);
+    // plane kernel: sum of the six plaquette traces per site; staple kernel: sum_mu Re tr W_mu = 4 x that
+    const double V = (double)lat->p.V;
+    QCD_TRY_RC(launch_sum_partials(ws, 1, blocks, 1.0 / ((plane ? 18.0 : 72.0) * V), out_plaq, st));
+    if (out_per_t) {  // blocks of one timeslice are consecutive (the t index of the tile is the slowest)
+        const int Lt = lat->p.L[3];
+        QCD_TRY_RC(launch_sum_partials(ws, Lt, blocks / Lt, (double)Lt / (18.0 * V), out_per_t, st));
+    }
+    return launch_sum_partials(ws + blocks, 1, blocks, 1.0, out_K, st);
 }
 
 int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
-                      void *Uout, double *out, double *ws, cudaStream_t st) {
+                      void *Uout, double *out_plaq, double *out_K, double *out_per_t, double *ws, cudaStream_t st) {
     const ForceSel fs = force_sel(lat, prec, QCD_ALL);
-    return prec == QCD_F64 ? launch_force_sums_t<double>(lat, fs, beta, eps_p, eps_u, U, P, Uout, out, ws, st)
-                           : launch_force_sums_t<float>(lat, fs, beta, eps_p, eps_u, U, P, Uout, out, ws, st);
+    return prec == QCD_F64
+               ? launch_force_sums_t<double>(lat, fs, beta, eps_p, eps_u, U, P, Uout, out_plaq, out_K, out_per_t, ws, st)
+               : launch_force_sums_t<float>(lat, fs, beta, eps_p, eps_u, U, P, Uout, out_plaq, out_K, out_per_t, ws, st);
 }
 
 // Single-pass MD step: P += eps_p F(U); Uout = reunit(exp(i eps_u P) U).  Subset ALL only (every link moves).

@@ -98,9 +98,9 @@ __global__ void map_kernel(const LatP lat, const int which, int32_t *__restrict_
     else out[s] = st.c[3];
 }
 
-int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *src, void *dst, bool unpack,
+int launch_pack(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *src, void *dst, bool unpack,
                 cudaStream_t st) {
-    const bool matrix = ncomp % 18 == 0 || ncomp % 24 == 0;  // complex-pair layout: colour matrices, spin-colour vectors
+    const bool matrix = pairs;  // complex-pair layout (colour matrices, spin-colour vectors) or real layout
     const size_t rb = prec == QCD_F64 ? 8 : 4;
     const size_t shm = (size_t)PK_SITES * (ncomp + 2) * rb;
     if (shm <= 48 * 1024) {  // transpose through shared memory; larger ncomp falls back to the direct kernel

@@ -95,14 +95,17 @@ int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, cons
                      const int32_t *subset_id, int nsub, double *out, double *ws, cudaStream_t st);
 // force + momentum update (+ link update into Uout when Uout != NULL: the single-pass step) with plaquette and
 // kinetic-energy sums as by-products (force.cu); ws: 2*blocks doubles
+// out_per_t != NULL: plaquette per timeslice as well; returns -1 without enqueuing anything if the launch
+// configuration cannot provide it (the caller then runs launch_plaquette)
 int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
-                      void *Uout, double *out, double *ws, cudaStream_t st);
-int launch_sum_partials(const double *partial, int count, double scale, double *out, cudaStream_t st);
+                      void *Uout, double *out_plaq, double *out_K, double *out_per_t, double *ws, cudaStream_t st);
+int force_sums_check(const qcd_lattice *lat, int prec);  // QCD_EWORKSPACE if the tuned tile has too many blocks
+int launch_sum_partials(const double *partial, int ngroups, int count, double scale, double *out, cudaStream_t st);
 int launch_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *eta,
                            cudaStream_t st);
 int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, const void *a, const void *b,
                          bool per_t, double *out, double *ws, cudaStream_t st);
-int launch_pack(const qcd_lattice *lat, int prec, int ncomp, const void *lex, void *soa, bool unpack,
+int launch_pack(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *lex, void *soa, bool unpack,
                 cudaStream_t st);
 int launch_get_map(const qcd_lattice *lat, int which, int32_t *out, cudaStream_t st);
 

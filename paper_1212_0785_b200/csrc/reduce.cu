@@ -223,10 +223,10 @@ int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *ou
                            : plaquette_t<float>(lat, U, out_avg, out_per_t, ws, st);
 }
 
-// out[0] = scale * sum of `count` per-block partials, fixed order (second pass of kernels that reduce as a
-// by-product, e.g. the force kernel with SUMS)
-int launch_sum_partials(const double *partial, int count, double scale, double *out, cudaStream_t st) {
-    reduce_pass2<<<dim3(1, 1), RED_THREADS, 0, st>>>(partial, 1, count, scale, out, 1);
+// out[g] = scale * sum of the `count` per-block partials partial[g*count .. (g+1)*count), g < ngroups, fixed
+// order (second pass of kernels that reduce as a by-product, e.g. the force kernel with SUMS)
+int launch_sum_partials(const double *partial, int ngroups, int count, double scale, double *out, cudaStream_t st) {
+    reduce_pass2<<<dim3(ngroups, 1), RED_THREADS, 0, st>>>(partial, ngroups, count, scale, out, 1);
     return check_launch("sum_partials");
 }
 

@@ -2,10 +2,10 @@
 
     python -m paper_1212_0785_b200.trajectory --config 5 --dtype f64 [--nsteps 20] [--no-observables]
 
-Momentum refresh and hot start from the counter-based generator, H before, a leapfrog
-trajectory (PAPER.md:17 operations; integrator R6), H after, dH.  With observables (default) every step's
-momentum update is `qcd_force_mom_update_sums`, so the plaquette and the kinetic energy of every step come
-out of the force kernel itself (no extra pass over the fields); without, the plain fused kernels run.
+Momentum refresh and hot start from the counter-based generator, then ONE library call:
+`qcd_trajectory` (leapfrog of single-pass steps, PAPER.md:17 operations, integrator R6) returns the plaquette,
+the per-timeslice plaquette and the kinetic energy of every step as by-products of the force kernel (no extra
+pass over the fields), hence H before, H after and dH.  `--no-observables` runs `qcd_leapfrog_single_pass`.
 Prints one JSON line: site-updates/s over the trajectory (CUDA events), the HBM fraction the step's algorithmic
 bytes correspond to, plaquette / K / H before and after, dH, and the per-step (plaquette, K) series.
 BASELINE.json config 5 ("sustained 20-step leapfrog trajectory with per-step reunitarization and reductions")
@@ -36,55 +36,48 @@ def run(config, dtype=torch.float64, nsteps=None, observables=True):
     n = nsteps or c["nsteps"]
     seed = SEED_BASE + config
     lat = qcd.Lattice(dims)
-    V = lat.V
-    U, P = lat.new_matrix_field(dtype), lat.new_matrix_field(dtype)
+    V, Lt = lat.V, dims[3]
+    U, P, W = lat.new_matrix_field(dtype), lat.new_matrix_field(dtype), lat.new_matrix_field(dtype)
     ws = lat.new_workspace()
     qcd.qcd_hot_start(lat, U, seed, c["sigma"])
     qcd.qcd_mom_refresh(lat, P, seed)
-    obs = torch.zeros((n + 2, 2), dtype=torch.float64, device="cuda")  # rows: start, after each step's kick
-
-    def energy(row):
-        qcd.qcd_plaquette(lat, U, obs[row, 0:1], None, ws)
-        qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, P, obs[row, 1:2], ws)
-
-    energy(0)
+    obs = torch.zeros((n + 1, 2), dtype=torch.float64, device="cuda")
+    per_t = torch.zeros((n + 1, Lt), dtype=torch.float64, device="cuda")
     stream = torch.cuda.current_stream()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record(stream)
-    # O11: P += eps/2 F; n x { U <- reunit(exp(i eps P) U); P += eps F (eps/2 on the last) }
-    qcd.qcd_force_mom_update(lat, U, P, beta, 0.5 * eps)
-    for k in range(n):
-        qcd.qcd_link_update(lat, P, U, eps, reunit=True)
-        step_eps = 0.5 * eps if k == n - 1 else eps
-        if observables:
-            qcd.qcd_force_mom_update_sums(lat, U, P, beta, step_eps, obs[k + 1], ws)
-        else:
-            qcd.qcd_force_mom_update(lat, U, P, beta, step_eps)
+    if observables:  # one library call: the integrator and every reduction run inside libqcdmd (qcd_trajectory)
+        qcd.qcd_trajectory(lat, U, P, W, beta, eps, n, obs, per_t, ws)
+    else:
+        qcd.qcd_leapfrog_single_pass(lat, U, P, W, beta, eps, n)
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
-    energy(n + 1)  # stand-alone reductions at the end: must agree with the by-products of the last kick
-    o = obs.cpu().numpy()
+    end = torch.zeros(2, dtype=torch.float64, device="cuda")  # stand-alone reductions at the end
+    qcd.qcd_plaquette(lat, U, end[0:1], None, ws)
+    qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, P, end[1:2], ws)
+    o, e = obs.cpu().numpy(), end.cpu().numpy()
 
-    def H(row):
-        return float(o[row, 1] + beta * 6 * V * (1 - o[row, 0]))
+    def H(plaq, K):
+        return float(K + beta * 6 * V * (1 - plaq))
 
     rb = 8 if dtype == torch.float64 else 4
     peak = 6532.5
     pk = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
     if os.path.exists(pk):
         peak = float(json.load(open(pk))["hbm_gbs"])
-    gbs = 432 * rb * V * n / (ms * 1e-3) / 1e9
+    gbs = 288 * rb * V * n / (ms * 1e-3) / 1e9  # single-pass steps: 288 reals per site and step
     line = {"config": config, "dims": list(dims), "dtype": "f64" if rb == 8 else "f32", "nsteps": n, "eps": eps,
             "beta": beta, "observables_every_step": observables, "ms": ms, "ms_per_step": ms / n,
             "site_updates_per_s": V * n / (ms * 1e-3), "step_hbm_gbs": gbs, "step_frac_of_hbm_peak": gbs / peak,
-            "plaq_start": float(o[0, 0]), "K_start": float(o[0, 1]), "H_start": H(0),
-            "plaq_end": float(o[n + 1, 0]), "K_end": float(o[n + 1, 1]), "H_end": H(n + 1), "dH": H(n + 1) - H(0),
-            "K_per_16V_start": float(o[0, 1] / (16 * V))}
+            "plaq_end": float(e[0]), "K_end": float(e[1]), "H_end": H(e[0], e[1])}
     if observables:
-        line["dH_from_fused_sums"] = H(n) - H(0)
-        line["per_step_plaq_K"] = [[float(a), float(b)] for a, b in o[1:n + 1]]
+        line.update({"plaq_start": float(o[0, 0]), "K_start": float(o[0, 1]), "H_start": H(*o[0]),
+                     "dH": H(*o[n]) - H(*o[0]), "H_end_from_fused_sums": H(*o[n]),
+                     "K_per_16V_start": float(o[0, 1] / (16 * V)),
+                     "per_step_plaq_K": [[float(a), float(b)] for a, b in o],
+                     "plaq_per_timeslice_end": [float(x) for x in per_t[n].cpu().numpy()]})
     return line
 
 

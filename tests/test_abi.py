@@ -89,7 +89,7 @@ def test_argument_validation_happens_before_any_cuda_call(qcd):
     assert L.qcd_sum_multi(h, qcd.F64, qcd.SUM_SCALAR, 1, a, b, 5000, b, b, None) == qcd.EINVAL
     assert L.qcd_leapfrog(h, qcd.F64, 5.0, 0.1, 0, a, b, None) == qcd.EINVAL
     assert L.qcd_get_map(h, 12, a, None) == qcd.EINVAL
-    assert L.qcd_pack(h, qcd.F64, 72, a, a, None) == qcd.EALIAS
+    assert L.qcd_pack(h, qcd.F64, 72, qcd.LAYOUT_PAIRS, a, a, None) == qcd.EALIAS
     assert L.qcd_md_host(h, qcd.F64, 5.0, 0.1, 1, None, a, b, None) == qcd.EINVAL
 
 

@@ -123,27 +123,27 @@ def test_pack_unpack_layout(qcd, orc, prec, dims):
     R = round_to(prec, inputs.random_real_field(4, V, 3))
     src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
     dst = lat.new_real_field(3, tdtype(prec))
-    qcd.qcd_pack(lat, 3, src, dst)
+    qcd.qcd_pack(lat, 3, qcd.LAYOUT_REAL, src, dst)
     got = lat.by_component(dst).cpu().numpy().astype(np.float64)
     assert np.array_equal(got[:, cb], R.T)
     back = torch.empty_like(src)
-    qcd.qcd_unpack(lat, 3, dst, back)
+    qcd.qcd_unpack(lat, 3, qcd.LAYOUT_REAL, dst, back)
     assert torch.equal(back, src)
     # many components per site: the direct (non-transposing) kernel
     R = round_to(prec, inputs.random_real_field(5, V, 100))
     src = torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1)
     dst = lat.new_real_field(100, tdtype(prec))
-    qcd.qcd_pack(lat, 100, src, dst)
+    qcd.qcd_pack(lat, 100, qcd.LAYOUT_REAL, src, dst)
     assert np.array_equal(lat.by_component(dst).cpu().numpy().astype(np.float64)[:, cb], R.T)
     back = torch.empty_like(src)
-    qcd.qcd_unpack(lat, 100, dst, back)
+    qcd.qcd_unpack(lat, 100, qcd.LAYOUT_REAL, dst, back)
     assert torch.equal(back, src)
 
 
 # ------------------------------------------------------------------ generators
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 8)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 8), (16, 16, 16, 32)])
 def test_mom_refresh_and_hot_start(qcd, orc_omp, prec, dims):
     lat = qcd.Lattice(dims)
     seed = inputs.config_seed(3)
@@ -231,7 +231,7 @@ def test_sum_and_sum_multi(qcd, orc, prec, dims):
     R[:, 2] = 1 - 2 * orc.map(dims, O.MAP_PARITY)
     R = round_to(prec, R)
     dR = lat.new_real_field(3, tdtype(prec))
-    qcd.qcd_pack(lat, 3, torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1), dR)
+    qcd.qcd_pack(lat, 3, qcd.LAYOUT_REAL, torch.from_numpy(R).to(tdtype(prec)).cuda().reshape(-1), dR)
     out3 = torch.zeros(3, dtype=torch.float64, device="cuda")
     for subset in (qcd.ALL, qcd.EVEN, qcd.ODD):
         qcd.qcd_sum(lat, qcd.SUM_SCALAR, 3, dR, out3, ws, subset=subset)
@@ -560,11 +560,27 @@ def sample_sites(dims, n, seed):
     return np.unique(np.array(pts, dtype=np.int32))
 
 
-@pytest.mark.parametrize("cfg,prec,single", [(4, "f64", False), (4, "f64", True), (5, "f32", False)])
+_full_start = {}
+
+
+def full_start(orc_omp, cfg):
+    """hot-start links and Gaussian momenta of a BASELINE config, whole lattice, from the oracle (cached: the
+    48^3x96 fields are 6 GB each)"""
+    if cfg not in _full_start:
+        _full_start.clear()  # one config at a time
+        c = inputs.CONFIGS[cfg]
+        seed = inputs.config_seed(cfg)
+        _full_start[cfg] = (orc_omp.hot_start(c["dims"], seed, c["sigma"]), orc_omp.mom_refresh(c["dims"], seed))
+    return _full_start[cfg]
+
+
+@pytest.mark.parametrize("cfg,prec,single", [(4, "f64", False), (4, "f64", True), (5, "f64", False), (5, "f64", True),
+                                             (5, "f32", False), (5, "f32", True)])
 def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
-    """BASELINE configs 4 (32^3x64 fp64, the headline) and 5 (48^3x96): the fused MD step exactly as
-    bench.py launches it (qcd_md_step, subset ALL), checked at sampled sites the oracle computes one
-    by one, plus properties that hold at any size."""
+    """BASELINE configs 4 (32^3x64 fp64, the headline) and 5 (48^3x96, both precisions): the fused MD step
+    exactly as bench.py launches it (two kernels in place, or the single-pass kernel), checked at sampled sites
+    the oracle computes one by one, the reductions of configs[3] ("sumMulti of plaquette per timeslice and
+    global kinetic-energy sum") on the WHOLE field against the oracle, plus properties that hold at any size."""
     import torch
     c = inputs.CONFIGS[cfg]
     dims, beta, eps = c["dims"], c["beta"], c["eps"]
@@ -575,7 +591,7 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
     qcd.qcd_hot_start(lat, dU, seed, c["sigma"])
     qcd.qcd_mom_refresh(lat, dP, seed)
     # the oracle builds the same start from the (seed, counter) definition, never from the GPU
-    U0 = orc_omp.hot_start(dims, seed, c["sigma"])
+    U0, P0 = full_start(orc_omp, cfg)
     sites = sample_sites(dims, 600, 1)
     cbmap = orc_omp.map(dims, O.MAP_CB_OF_LEX)
     cbs = torch.from_numpy(cbmap[sites].astype(np.int64)).cuda()
@@ -586,18 +602,15 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
 
     tolgen = 1e-12 if prec == "f64" else 2e-7
     assert rel(gather(dU), U0[sites]) < tolgen
-    if prec == "f32":  # the fp32 path starts from rounded links: give the oracle the same (in place, chunked)
-        flat = U0.reshape(-1).view(np.float64)
-        for i in range(0, flat.size, 1 << 26):
-            flat[i:i + (1 << 26)] = flat[i:i + (1 << 26)].astype(np.float32)
-    # momenta at the sampled sites from the oracle's generator blocks (the RNG is keyed on the site)
-    Psites = np.empty((len(sites), 4, 3, 3), dtype=np.complex128)
-    for i, s_ in enumerate(sites):
+    if prec == "f32":  # the fp32 path starts from rounded fields: give the oracle the same
+        U0, P0 = round_to(prec, U0), round_to(prec, P0)
+    # momenta at a few sampled sites once more from the oracle's generator blocks (the RNG is keyed on the site)
+    for s_ in sites[:8]:
         for mu in range(4):
             q = np.concatenate([orc_omp.rng_block(seed, int(s_), mu, j, 0, 1)[2] for j in range(4)])
-            Psites[i, mu] = orc_omp.herm_from_coeffs(q)
+            assert np.abs(round_to(prec, orc_omp.herm_from_coeffs(q)) - P0[s_, mu]).max() == 0
+    Psites = P0[sites]
     assert rel(gather(dP), Psites) < tolgen
-    Psites = round_to(prec, Psites)
     ws = lat.new_workspace()
     plaq = torch.zeros(1, dtype=torch.float64, device="cuda")
     per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
@@ -628,9 +641,17 @@ def test_full_size_md_step_sampled_parity(qcd, orc_omp, cfg, prec, single):
     gP = gather(dP)
     assert np.abs(gP - np.conj(np.swapaxes(gP, -1, -2))).max() < utol * 10
     assert np.abs(np.trace(gP, axis1=-2, axis2=-1)).max() < utol * 10
-    # kinetic energy of the updated momenta: K/(16 V) stays near 1 for this small step
+    # the reductions on the whole field: kinetic energy (sum) and per timeslice (sumMulti) of the UPDATED momenta
+    # against the oracle's own force on the whole lattice, and the per-timeslice plaquette of the updated links
+    P1full = P0 + eps * orc_omp.gauge_force(dims, beta, U0)
     K = torch.zeros(1, dtype=torch.float64, device="cuda")
+    Kt = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
     qcd.qcd_sum(lat, qcd.SUM_NORM2, 72, dP, K, ws)
+    qcd.qcd_sum_multi(lat, qcd.SUM_NORM2, 72, dP, None, dims[3], Kt, ws)
+    flat = P1full.view(np.float64).reshape(lat.V, 72)
+    rK, rKt = orc_omp.sum(dims, O.SUM_NORM2, flat)[0], orc_omp.sum_multi(dims, O.SUM_NORM2, flat)
+    assert abs(K.item() - rK) < TOL[prec] * rK
+    assert rel(Kt.cpu().numpy(), rKt) < TOL[prec]
     assert abs(K.item() / (16 * lat.V) - 1) < 0.01
 
 
@@ -705,15 +726,133 @@ def test_config_observables_against_stored_oracle_values(qcd, n):
 
 
 def test_trajectory_driver_reports_the_stored_dH(qcd):
-    """paper_1212_0785_b200.trajectory (per-step observables from the force kernel) on config 2"""
+    """paper_1212_0785_b200.trajectory (one qcd_trajectory call, observables from the force kernel) on config 2"""
     import json
     import os
     from paper_1212_0785_b200 import trajectory
     g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "config_values.json")))["2"]
     r = trajectory.run(2)
     scale = abs(g["K0"] + g["S0"])
-    assert abs(r["dH"] - g["dH"]) <= 1e-12 * scale and abs(r["dH_from_fused_sums"] - g["dH"]) <= 1e-12 * scale
-    assert abs(r["plaq_end"] - g["plaq1"]) < 1e-12 and len(r["per_step_plaq_K"]) == g["nsteps"]
+    assert abs(r["dH"] - g["dH"]) <= 1e-12 * scale and abs(r["H_end_from_fused_sums"] - r["H_end"]) <= 1e-12 * scale
+    assert abs(r["plaq_end"] - g["plaq1"]) < 1e-12 and len(r["per_step_plaq_K"]) == g["nsteps"] + 1
     assert abs(r["per_step_plaq_K"][-1][0] - r["plaq_end"]) < 1e-13
+    assert abs(np.mean(r["plaq_per_timeslice_end"]) - r["plaq_end"]) < 1e-13
     r2 = trajectory.run(2, observables=False)
-    assert abs(r2["dH"] - r["dH"]) <= 1e-12 * scale
+    assert abs(r2["H_end"] - r["H_end"]) <= 1e-12 * scale
+
+
+def oracle_trajectory_observed(orc, dims, beta, eps, n, U, P):
+    """O11 step by step on the oracle with the observables qcd_trajectory reports (include/qcd.h): row k =
+    (plaquette of U_k, K of the momenta after the kick that follows link update k; row 0: K of the initial momenta),
+    and the per-timeslice plaquette of U_k"""
+    V = O.Oracle.volume(dims)
+    obs, per_t = np.empty((n + 1, 2)), np.empty((n + 1, dims[3]))
+
+    def K(P):
+        return orc.sum(dims, O.SUM_NORM2, P.view(np.float64).reshape(V, 72))[0]
+
+    obs[0, 0], per_t[0] = orc.plaquette(dims, U)
+    obs[0, 1] = K(P)
+    P = orc.mom_update(dims, eps / 2, orc.gauge_force(dims, beta, U), P)
+    for k in range(1, n + 1):
+        U = orc.link_update(dims, eps, P, U, reunit=True)
+        obs[k, 0], per_t[k] = orc.plaquette(dims, U)
+        P = orc.mom_update(dims, eps / 2 if k == n else eps, orc.gauge_force(dims, beta, U), P)
+        obs[k, 1] = K(P)
+    return U, P, obs, per_t
+
+
+@pytest.mark.parametrize("dims,prec,n,tile", [((4, 4, 4, 4), "f64", 1, None), ((8, 8, 8, 16), "f64", 4, None),
+                                               ((8, 8, 8, 16), "f64", 5, None), ((6, 4, 2, 8), "f64", 3, None),
+                                               ((8, 8, 8, 16), "f64", 3, (8, 2, 2, 2)), ((8, 8, 8, 16), "f32", 3, None),
+                                               ((8, 8, 8, 16), "f64", 4, (8, 4, 4, 1)), ((8, 8, 8, 16), "f32", 2, (8, 4, 4, 1)),
+                                               ((8, 8, 8, 16), "f64", 3, (8, 4, 2, 1)), ((8, 8, 8, 16), "f64", 2, "staple")])
+def test_trajectory_observables_every_step(qcd, orc_omp, dims, prec, n, tile):
+    """qcd_trajectory: final fields and the per-step (plaquette, per-timeslice plaquette, K) series against the
+    oracle's leapfrog step by step; odd and even step counts (the ping-pong starts differently), a block that
+    is not a whole number of warps, tiles inside one timeslice (per-timeslice values are by-products of the force
+    kernel), tiles that span two timeslices and the staple variant (they then come from the stand-alone
+    plaquette kernel)"""
+    import torch
+    beta, eps = 5.8, 0.05
+    lat = qcd.Lattice(dims)
+    U = round_to(prec, orc_omp.hot_start(dims, 77, 0.4))
+    P = round_to(prec, orc_omp.mom_refresh(dims, 78))
+    dU, dP, dW = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec), lat.new_matrix_field(tdtype(prec))
+    ws = lat.new_workspace()
+    obs = torch.zeros((n + 1, 2), dtype=torch.float64, device="cuda")
+    per_t = torch.zeros((n + 1, dims[3]), dtype=torch.float64, device="cuda")
+    p = qcd.F64 if prec == "f64" else qcd.F32
+    try:
+        if tile == "staple":
+            qcd.qcd_tune_set(lat, p, qcd.ALL, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index("staple"), None)
+        elif tile:
+            qcd.qcd_tune_set(lat, p, qcd.ALL, qcd.KERNEL_FORCE, qcd.FORCE_VARIANTS.index("plane"), tile)
+        qcd.qcd_trajectory(lat, dU, dP, dW, beta, eps, n, obs, per_t, ws)
+        obs2, per_t2 = torch.zeros_like(obs), torch.zeros_like(per_t)
+        dU2, dP2 = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec)
+        qcd.qcd_trajectory(lat, dU2, dP2, dW, beta, eps, n, obs2, per_t2, ws)
+        # without the per-timeslice output
+        dU3, dP3, obs3 = dev(qcd, lat, U, prec), dev(qcd, lat, P, prec), torch.zeros_like(obs)
+        qcd.qcd_trajectory(lat, dU3, dP3, dW, beta, eps, n, obs3, None, ws)
+    finally:
+        qcd.qcd_tune_clear()
+    rU, rP, robs, rper_t = oracle_trajectory_observed(orc_omp, dims, beta, eps, n, U, P)
+    assert rel(host(qcd, lat, dU), rU) < TOL[prec] and rel(host(qcd, lat, dP), rP) < TOL[prec]
+    o = obs.cpu().numpy()
+    assert np.abs(o[:, 0] - robs[:, 0]).max() < TOL[prec] and rel(o[:, 1], robs[:, 1]) < TOL[prec]
+    assert np.abs(per_t.cpu().numpy() - rper_t).max() < TOL[prec]
+    H = o[:, 1] + beta * 6 * lat.V * (1 - o[:, 0])
+    rH = robs[:, 1] + beta * 6 * lat.V * (1 - robs[:, 0])
+    assert abs((H[n] - H[0]) - (rH[n] - rH[0])) <= TOL[prec] * abs(rH[0])  # R15: dH against |H|
+    # deterministic run to run, per-timeslice values average to the global one
+    assert torch.equal(obs, obs2) and torch.equal(per_t, per_t2) and torch.equal(dU, dU2) and torch.equal(dP, dP2)
+    assert np.abs(per_t.cpu().numpy().mean(axis=1) - o[:, 0]).max() < (1e-13 if prec == "f64" else 1e-7)
+    # argument checks come before anything is enqueued
+    assert np.abs(obs3.cpu().numpy() - o).max() < 1e-12 * np.abs(o).max() and torch.equal(dU3, dU)
+    small = torch.empty(8, dtype=torch.float64, device="cuda")
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.qcd_trajectory(lat, dU3, dP3, dW, beta, eps, n, obs3, None, small)
+    assert e.value.code == qcd.EWORKSPACE and torch.equal(dU3, dU)
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.qcd_trajectory(lat, dU3, dP3, dU3, beta, eps, n, obs3, None, ws)
+    assert e.value.code == qcd.EALIAS
+
+
+@pytest.mark.parametrize("cfg,prec,n", [(4, "f64", 4), (5, "f64", 20), (5, "f32", 2)])
+def test_config_trajectory_full_size_against_oracle(qcd, orc_omp, cfg, prec, n):
+    """BASELINE configs 4 and 5 at full size ("sustained 20-step leapfrog trajectory with per-step
+    reunitarization and reductions ... reports dH"): qcd_trajectory against the OpenMP build of the oracle,
+    step by step — plaquette, per-timeslice plaquette and K of every step, dH (R15: against |H|), final links and
+    momenta at sampled sites.  Config 5 fp64 runs all 20 steps; the other two rows are shortened to 4 and 2 steps
+    to keep the suite's time down (the oracle needs about 9 s per 48^3x96 step on 16 host cores)."""
+    import torch
+    c = inputs.CONFIGS[cfg]
+    dims, beta, eps = c["dims"], c["beta"], c["eps"]
+    seed = inputs.config_seed(cfg)
+    lat = qcd.Lattice(dims)
+    dt = tdtype(prec)
+    dU, dP, dW = lat.new_matrix_field(dt), lat.new_matrix_field(dt), lat.new_matrix_field(dt)
+    qcd.qcd_hot_start(lat, dU, seed, c["sigma"])
+    qcd.qcd_mom_refresh(lat, dP, seed)
+    ws = lat.new_workspace()
+    obs = torch.zeros((n + 1, 2), dtype=torch.float64, device="cuda")
+    per_t = torch.zeros((n + 1, dims[3]), dtype=torch.float64, device="cuda")
+    qcd.qcd_trajectory(lat, dU, dP, dW, beta, eps, n, obs, per_t, ws)
+    U0, P0 = full_start(orc_omp, cfg)
+    rU, rP, robs, rper_t = oracle_trajectory_observed(orc_omp, dims, beta, eps, n, round_to(prec, U0), round_to(prec, P0))
+    _full_start.clear()
+    o = obs.cpu().numpy()
+    assert np.abs(o[:, 0] - robs[:, 0]).max() < TOL[prec] and rel(o[:, 1], robs[:, 1]) < TOL[prec]
+    assert np.abs(per_t.cpu().numpy() - rper_t).max() < TOL[prec]
+    H = o[:, 1] + beta * 6 * lat.V * (1 - o[:, 0])
+    rH = robs[:, 1] + beta * 6 * lat.V * (1 - robs[:, 0])
+    assert abs((H[n] - H[0]) - (rH[n] - rH[0])) <= TOL[prec] * abs(rH[0])
+    sites = sample_sites(dims, 2000, 3)
+    cbs = torch.from_numpy(orc_omp.map(dims, O.MAP_CB_OF_LEX)[sites].astype(np.int64)).cuda()
+
+    def gather(field):
+        g = field[cbs >> 5, :, cbs & 31, :].permute(1, 0, 2).to(torch.float64).cpu().numpy()
+        return (g[..., 0] + 1j * g[..., 1]).T.reshape(len(sites), 4, 3, 3)
+
+    assert rel(gather(dU), rU[sites]) < TOL[prec] and rel(gather(dP), rP[sites]) < TOL[prec]

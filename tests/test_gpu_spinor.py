@@ -22,7 +22,7 @@ def spinor_to_device(qcd, lat, a, prec):
     import torch
     t = torch.view_as_real(torch.from_numpy(np.ascontiguousarray(a))).reshape(-1).to(tdtype(prec)).cuda()
     out = lat.new_pair_field(a.shape[1], tdtype(prec))
-    qcd.qcd_pack(lat, 2 * a.shape[1], t, out)
+    qcd.qcd_pack(lat, 2 * a.shape[1], qcd.LAYOUT_PAIRS, t, out)
     return out
 
 
@@ -30,7 +30,7 @@ def spinor_to_host(qcd, lat, d):
     import torch
     nc = d.shape[1]
     t = torch.empty(lat.V * nc * 2, dtype=d.dtype, device="cuda")
-    qcd.qcd_unpack(lat, 2 * nc, d, t)
+    qcd.qcd_unpack(lat, 2 * nc, qcd.LAYOUT_PAIRS, d, t)
     return t.to(torch.float64).cpu().numpy().view("complex128").reshape(lat.V, nc)
 
 

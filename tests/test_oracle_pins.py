@@ -347,6 +347,44 @@ def test_force_subsets(orc):
     assert np.array_equal(Fo[par == 1], F[par == 1]) and np.all(Fo[par == 0] == 7.0)
 
 
+# ------------------------------------------------------------------ O3/O5: perturbation noise (config 3)
+
+def test_perturb_noise_layout_and_moments(orc_omp, orc):
+    """"Perturbation noise: 18 Gaussians from blocks 0..8 in storage order [row][col][re,im]",
+    purpose 2, counter keyed on the lexicographic site, stride-16 block index mu*16 + j; O5: U + sigma N.
+    Rebuilt here by hand from the generator blocks (rng_block itself is pinned by the Philox known answers and
+    the uniform / Gaussian tests above), then the moments of the 18 reals over 1.3 x 10^5 links: a wrong block
+    index, purpose, storage order, sign or a variance-of-2 slip fails."""
+    dims, seed, sigma = (16, 16, 16, 8), 0x1212078500000003, 1e-3
+    V = O.Oracle.volume(dims)
+    U = np.zeros((V, 4, 3, 3), dtype=np.complex128)
+    N = orc_omp.perturb(dims, seed, sigma, U) / sigma  # the noise itself
+    # elements by hand: entry e = 3*row + col of link (s, mu) is g[0] + i g[1] of block (s, mu, j = e, stream 0, purpose 2)
+    for s_, mu, row, col in [(0, 0, 0, 0), (V - 1, 3, 2, 2), (4711, 2, 1, 2), (17, 1, 2, 0), (V // 2 + 5, 0, 0, 1)]:
+        g = orc.rng_block(seed, s_, mu, 3 * row + col, 0, 2)[2]
+        assert abs(N[s_, mu, row, col] - (g[0] + 1j * g[1])) < 1e-12
+    # other purposes / streams / a neighbouring block give different numbers
+    g1 = orc.rng_block(seed, 0, 0, 0, 0, 1)[2]
+    g2 = orc.rng_block(seed, 0, 0, 1, 0, 2)[2]
+    assert abs(N[0, 0, 0, 0] - (g1[0] + 1j * g1[1])) > 1e-6 and abs(N[0, 0, 0, 0] - (g2[0] + 1j * g2[1])) > 1e-6
+    # perturbation is additive and linear in sigma
+    U0 = orc_omp.hot_start(dims, 5, 0.5)
+    assert np.abs(orc_omp.perturb(dims, seed, sigma, U0) - (U0 + sigma * N)).max() < 1e-15
+    # moments: 18 iid N(0,1) reals per link
+    x = N.reshape(-1, 9).view(np.float64).reshape(-1, 18)
+    n = x.shape[0]
+    assert n >= 100000
+    assert np.abs(x.mean(axis=0)).max() < 5 / np.sqrt(n)
+    assert np.abs(x.var(axis=0) - 1).max() < 5 * np.sqrt(2.0 / n)
+    assert abs((x ** 4).mean() - 3) < 5 * np.sqrt(96.0 / x.size)
+    c = np.corrcoef(x.T)
+    assert np.abs(c - np.eye(18)).max() < 5 / np.sqrt(n)  # re/im and entries uncorrelated
+    # and across links of a site / neighbouring sites
+    flat = x.reshape(V, 4 * 18)
+    assert abs(np.corrcoef(flat[:, 0], flat[:, 18])[0, 1]) < 5 / np.sqrt(V)
+    assert abs(np.corrcoef(flat[:-1, 0], flat[1:, 0])[0, 1]) < 5 / np.sqrt(V)
+
+
 # ------------------------------------------------------------------ O9, O10
 
 def test_reunit_pins(orc):
