@@ -6,7 +6,7 @@
 A "step" is one fused molecular-dynamics step on the whole lattice: P += eps F(U), then
 U <- reunit(exp(i eps P) U) — force, projection, momentum update, exponential, link update and
 reunitarisation, all rows of SURVEY.md section 8(a)'s MD step.  --path single_pass (default, the faster one as
-measured: profiles/r01d_*.md) runs it as ONE kernel, qcd_md_step_single_pass, ping-ponging two gauge fields
+measured: profiles/r02_*.md) runs it as ONE kernel, qcd_md_step_single_pass, ping-ponging two gauge fields
 (8(a) "MD step (single pass)", 288 reals/site); --path two_kernel as qcd_force_mom_update followed by
 qcd_link_update(reunit) in place (8(a) "MD step (fused)", 432 reals/site).  Default workload: BASELINE
 config 4, 32^3x64 fp64, sigma=0.2, beta=6.0, eps=0.02, seeded synthetic hot start generated on the device.
@@ -37,6 +37,11 @@ CONFIGS = {  # BASELINE.json configs: dims, hot-start sigma, beta, eps
 # reals/site R+W: force+mom reads U,P writes P; exp+reunit reads P,U writes U; the single-pass
 # kernel reads U,P and writes P,U
 BYTES_PER_SITE = {"force_mom_update": 216, "link_update_reunit": 216, "md_step_single_pass": 288}
+# FP64/FP32 arithmetic instructions per site of the default kernels: the plane-sharing force is
+# 6 planes x (108 + 108 + 90) + 12 down staples x 216 + 4 x 90 (U_mu A, TA part only) = 4788 FMA, + projection and
+# P += eps F; the link update is about 480 per link (Hermitian Q^2 54, series ~95, two rows of E 40, two rows of
+# E U 72, reunit ~100, norm, scaling, det ~70)
+FMA_FORCE, FMA_MOM, FMA_LINK = 4788, 112, 4 * 480
 METRIC = "md_step_site_updates_per_s"
 UNIT = "site-updates/s"
 
@@ -204,6 +209,12 @@ def run_ours(args, cfg):
             if ev:
                 ev[2].record(stream)
 
+    # the FMA denominator: register-resident 3x3 complex product chains, measured now
+    prec = qcd.F64 if args.dtype == "f64" else qcd.F32
+    fma_peak = qcd.probe_rate(qcd.PROBE_FMA, prec)
+    fma_src = "measured in this run: qcd_probe_launch(QCD_PROBE_FMA), best of 3, CUDA events"
+    time.sleep(0.5)  # let the board cool off the probe before the timed region
+
     nwarm = args.warmup + (args.warmup & 1 if single else 0)  # even, so the timed steps start from bufs[0]
     for k in range(nwarm):
         step(k)
@@ -227,6 +238,26 @@ def run_ours(args, cfg):
     force_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / K
     link_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / K
     value, elapsed_ms = aggregate(elapsed_ms, V, K, world, "cuda")
+    clocks_timed = sampler.summary()
+
+    # ---- the sustained regime (a trajectory lives there: the fp64 step draws the board's full power and the driver
+    # lowers the SM clock after a few tenths of a second): a second, longer loop outside the --steps region
+    sustained = None
+    if args.sustained_steps > 0:
+        Ks = args.sustained_steps + (args.sustained_steps & 1 if single else 0)
+        sampler.samples, sampler.mask = [], 0
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        sampler.active = True
+        s0.record(stream)
+        for k in range(Ks):
+            step(k)
+        s1.record(stream)
+        barrier()
+        sampler.active = False
+        _, sus_ms = aggregate(s0.elapsed_time(s1), V, Ks, world, "cuda")
+        sustained = {"steps": Ks, "ms_per_step": sus_ms / Ks, "site_updates_per_s": world * V * Ks / (sus_ms * 1e-3),
+                     "clocks": sampler.summary()}
 
     # ---- e2e: the C-ABI call on HOST buffers (pinned), H2D + pack + step + unpack + D2H every step
     Ke = max(1, min(K, args.e2e_steps))
@@ -279,17 +310,21 @@ def run_ours(args, cfg):
                    "step_hbm_gbs": step_bytes / (elapsed_ms / K * 1e-3) / 1e9,
                    "step_frac_of_hbm_peak": step_bytes / (elapsed_ms / K * 1e-3) / 1e9 / peak,
                    "kernel_ms": {top: force_ms} if single else
-                                {"force_mom_update": force_ms, "link_update_reunit": link_ms}},
+                                {"force_mom_update": force_ms, "link_update_reunit": link_ms},
+                   "sustained": sustained},
         "roofline": {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": force_bytes,
+                     "traffic_source": "stored ncu capture (profiles/roofline_traffic.json names the report), not measured in this run",
                      # the same kernel against the plain-ALU roofline it also sits near: FMA per site x V
-                     # / time over the nominal 148 SMs x 64 (fp64) or 128 (fp32) lanes x 1.965 GHz
-                     "fma_frac": (5616 + 222 + (4 * 550 if single else 0)) * V / (force_ms * 1e-3) / FMA_PEAK[args.dtype]},
+                     # / time over the FMA rate the qcd_probe_launch(QCD_PROBE_FMA) kernel reached a moment ago
+                     "fma_frac": (FMA_FORCE + FMA_MOM + (FMA_LINK if single else 0)) * V / (force_ms * 1e-3) / fma_peak,
+                     "fma_per_site": FMA_FORCE + FMA_MOM + (FMA_LINK if single else 0),
+                     "fma_peak": fma_peak, "fma_peak_source": fma_src},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * fb, "d2h_bytes_per_step": 2 * fb,
                 "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout)"},
         "gpu_launches": K if single else 2 * K,
-        "clocks": sampler.summary(),
+        "clocks": clocks_timed,
     }
     if world == 1 and not args.no_cpu_baseline:
         from oracle.oracle import Oracle
@@ -315,20 +350,41 @@ def run_ours(args, cfg):
 # per-kernel table: reals per site read + written, FMA per site (products x 108 + small)
 KERNEL_TABLE = [
     # name, reals/site, FMA/site, subsets
-    ("gauge_force", 144, 5616 + 150, True),
+    ("gauge_force", 144, FMA_FORCE + 40, True),
     ("mom_update", 216, 72, True),
-    ("force_mom_update", 216, 5616 + 222, True),
-    ("link_update", 216, 4 * 410, True),
-    ("reunit", 144, 4 * 150, True),
-    ("link_update_reunit", 216, 4 * 550, True),
+    ("force_mom_update", 216, FMA_FORCE + FMA_MOM, True),
+    ("link_update", 216, 4 * 420, True),
+    ("reunit", 144, 4 * 100, True),
+    ("link_update_reunit", 216, FMA_LINK, True),
     ("mom_refresh", 72, 0, True),
     ("plaquette", 72, 12 * 108 + 6 * 18, False),
     ("sum_norm2", 72, 72, True),
     ("sum_multi_norm2_per_t", 72, 72, False),
-    ("md_step_single_pass", 288, 5616 + 222 + 4 * 550, False),
-    ("force_mom_update_sums", 216, 5616 + 330, False),
+    ("md_step_single_pass", 288, FMA_FORCE + FMA_MOM + FMA_LINK, False),
+    ("force_mom_update_sums", 216, FMA_FORCE + FMA_MOM + 180, False),
 ]
-FMA_PEAK = {"f64": 148 * 64 * 1.965e9, "f32": 148 * 128 * 1.965e9}  # nominal lanes x clock
+FMA_PEAK_NOMINAL = {"f64": 148 * 64 * 1.965e9, "f32": 148 * 128 * 1.965e9}  # lanes x clock
+
+
+def run_peaks(args):
+    """the measured denominators: FMA (fp64, fp32), L1-resident loads, shared memory, L2-resident loads"""
+    import torch
+
+    from paper_1212_0785_b200 import binding as qcd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    out = {"device": torch.cuda.get_device_name(0), "sms": sms}
+    for name, what, prec in (("fma_f64_per_s", qcd.PROBE_FMA, qcd.F64), ("fma_f32_per_s", qcd.PROBE_FMA, qcd.F32),
+                             ("l1_resident_ldg128_bytes_per_s", qcd.PROBE_L1, qcd.F64),
+                             ("shared_lds128_bytes_per_s", qcd.PROBE_LDS, qcd.F64),
+                             ("l2_resident_ldg128_bytes_per_s", qcd.PROBE_L2, qcd.F64)):
+        time.sleep(0.5)
+        out[name] = qcd.probe_rate(what, prec)
+    out["nominal_fma_per_s"] = FMA_PEAK_NOMINAL
+    out["l1_bytes_per_clk_per_sm_at_1965MHz"] = out["l1_resident_ldg128_bytes_per_s"] / sms / 1.965e9
+    out["lds_bytes_per_clk_per_sm_at_1965MHz"] = out["shared_lds128_bytes_per_s"] / sms / 1.965e9
+    print(json.dumps({"peaks": out, "how": "qcd_probe_launch through the C ABI, CUDA events, best of 3 per probe"}), flush=True)
 
 
 def run_per_kernel(args, cfg):
@@ -350,6 +406,7 @@ def run_per_kernel(args, cfg):
     per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")  # 4 x L2
     peak, peak_src = peaks()
+    fma_peak = qcd.probe_rate(qcd.PROBE_FMA, qcd.F64 if args.dtype == "f64" else qcd.F32)
     stream = torch.cuda.current_stream()
 
     def reset():
@@ -397,10 +454,11 @@ def run_per_kernel(args, cfg):
             gbs = reals * rb * sites / (ms * 1e-3) / 1e9
             rows.append({"kernel": name, "subset": sname, "ms": ms, "bytes_per_site": reals * rb, "gbs": gbs,
                          "frac_hbm": gbs / peak, "site_updates_per_s": sites / (ms * 1e-3),
-                         "frac_fma": fma * sites / (ms * 1e-3) / FMA_PEAK[args.dtype]})
+                         "frac_fma": fma * sites / (ms * 1e-3) / fma_peak})
     print(json.dumps({"per_kernel": rows, "config": {"workload": f"{cfg['name']} {args.dtype}, each kernel alone, "
                       "L2 flushed (512 MB write) before every timed launch", "reps": reps},
-                      "peak_gbs": peak, "peak_source": peak_src, "fma_peak": FMA_PEAK[args.dtype]}), flush=True)
+                      "peak_gbs": peak, "peak_source": peak_src, "fma_peak": fma_peak,
+                      "fma_peak_source": "qcd_probe_launch(QCD_PROBE_FMA), measured in this run"}), flush=True)
 
 
 def main():
@@ -415,6 +473,10 @@ def main():
                     help="single_pass (default, the faster one as measured): qcd_md_step_single_pass ping-ponging two "
                          "gauge fields; two_kernel: qcd_force_mom_update + qcd_link_update(reunit) in place")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--sustained-steps", type=int, default=600,
+                    help="length of the second timed loop that reports the power-capped regime (0: skip)")
+    ap.add_argument("--peaks", action="store_true",
+                    help="measure the FMA / L1 / shared-memory / L2 denominators with the library's probe kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-kernel", action="store_true",
                     help="instead of the MD-step line: every kernel alone on ALL/EVEN/ODD with an L2 flush between "
@@ -424,6 +486,8 @@ def main():
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.peaks:
+        run_peaks(args)
     elif args.per_kernel:
         run_per_kernel(args, cfg)
     else:

@@ -306,6 +306,21 @@ int qcd_perturb(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, v
 int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, const uint32_t *site,
                    const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, void *stream);
 
+/* ---- measured denominators ("Measure DFMA/FFMA peaks with a probe") --------------------
+ * One kernel launch per probe, enqueued on `stream` like every other call and timed by the caller with CUDA
+ * events (bench.py --peaks): rate = qcd_probe_work(...) / elapsed.
+ *   QCD_PROBE_FMA  chains of 3x3 complex products in registers (the product routine of the force kernel), no
+ *                  memory traffic: work = real FMAs.  prec selects double / float.
+ *   QCD_PROBE_L1   every block re-reads its own 32 kB with 128-bit loads: work = bytes (L1-resident loads)
+ *   QCD_PROBE_LDS  the same from 64 kB of shared memory: work = bytes
+ *   QCD_PROBE_L2   all blocks stream one 48 MB buffer: work = bytes (L2-resident as the SMs see it)
+ * scratch: device memory, qcd_probe_scratch_bytes(what) bytes, zero-filled by the caller; QCD_EWORKSPACE if
+ * smaller.  qcd_probe_work and qcd_probe_scratch_bytes are host-only. */
+enum { QCD_PROBE_FMA = 0, QCD_PROBE_L1 = 1, QCD_PROBE_LDS = 2, QCD_PROBE_L2 = 3 };
+size_t qcd_probe_scratch_bytes(int what);
+double qcd_probe_work(int what, int prec, int reps);
+int qcd_probe_launch(int what, int prec, int reps, void *scratch, size_t scratch_bytes, void *stream);
+
 /* End-to-end call on HOST buffers (used for the e2e measurement): U_host and P_host are host arrays
  * in the canonical layout (pinned memory makes the copies asynchronous).  Enqueues on `stream`:
  * host->device copies, pack, `nsteps` fused MD steps (eps_p = eps_u = eps), unpack, device->host

@@ -16,6 +16,7 @@ F32, F64 = 0, 1
 ALL, EVEN, ODD = 0, 1, 2
 SUM_SCALAR, SUM_NORM2, SUM_RETR = 0, 1, 2
 LAYOUT_REAL, LAYOUT_PAIRS = 0, 1
+PROBE_FMA, PROBE_L1, PROBE_LDS, PROBE_L2 = 0, 1, 2, 3
 OK, EINVAL, EDIMS, EALIGN, EALIAS, EWORKSPACE, ECUDA = range(7)
 KERNEL_FORCE, KERNEL_LINK_UPDATE, KERNEL_MOM_UPDATE = 0, 1, 2
 FORCE_VARIANTS = ("staple", "plane")  # index = QCD_FORCE_* value
@@ -65,6 +66,9 @@ SIGNATURES = {
     "qcd_hot_start": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
     "qcd_perturb": (_i, [_vp, _i, _u64, _d, _vp, _vp]),
     "qcd_rng_blocks": (_i, [_u64, _u32, _u32, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_probe_scratch_bytes": (_sz, [_i]),
+    "qcd_probe_work": (_d, [_i, _i, _i]),
+    "qcd_probe_launch": (_i, [_i, _i, _i, _vp, _sz, _vp]),
     "qcd_md_host": (_i, [_vp, _i, _d, _d, _i, _vp, _vp, _vp, _vp]),
 }
 
@@ -329,6 +333,27 @@ def qcd_md_host(lat, U_host, P_host, beta, eps, nsteps, device_work, stream=None
     """U_host, P_host: host tensors (pinned for asynchronous copies) in the canonical layout [V,4,3,3,2]."""
     _check(lib.qcd_md_host(lat.handle, _prec(U_host), beta, eps, nsteps, _ptr(U_host), _ptr(P_host),
                            _ptr(device_work), _stream(stream)))
+
+
+def qcd_probe_launch(what, prec, reps, scratch, stream=None):
+    _check(lib.qcd_probe_launch(what, prec, reps, _ptr(scratch), scratch.numel() * scratch.element_size(),
+                                _stream(stream)))
+
+
+def probe_rate(what, prec=F64, reps=None):
+    """work per second of one probe launch (FMA/s or bytes/s), CUDA events, best of 3 after a warm-up"""
+    reps = reps or {PROBE_FMA: 4000, PROBE_L1: 2000, PROBE_LDS: 4000, PROBE_L2: 20}[what]
+    scratch = torch.zeros(lib.qcd_probe_scratch_bytes(what) // 8 + 1, dtype=torch.float64, device="cuda")
+    qcd_probe_launch(what, prec, max(1, reps // 50), scratch)
+    best = float("inf")
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        qcd_probe_launch(what, prec, reps, scratch)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    return lib.qcd_probe_work(what, prec, reps) / (best * 1e-3)
 
 
 # ---- convenience used by tests and bench: canonical host arrays <-> device fields (via qcd_pack) ----

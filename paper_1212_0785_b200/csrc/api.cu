@@ -583,6 +583,25 @@ int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, c
     return launch_rng_blocks(seed, stream_id, purpose, n, site, mu_j, words, uniforms, gauss, (cudaStream_t)stream);
 }
 
+size_t qcd_probe_scratch_bytes(int what) {
+    return what >= QCD_PROBE_FMA && what <= QCD_PROBE_L2 ? probe_scratch_bytes(what) : 0;
+}
+
+double qcd_probe_work(int what, int prec, int reps) {
+    if (what < QCD_PROBE_FMA || what > QCD_PROBE_L2 || reps < 1) return 0.0;
+    return probe_work(what, prec, reps);
+}
+
+int qcd_probe_launch(int what, int prec, int reps, void *scratch, size_t scratch_bytes, void *stream) {
+    const char *fn = "qcd_probe_launch";
+    if (what < QCD_PROBE_FMA || what > QCD_PROBE_L2) return bad(QCD_EINVAL, "%s: unknown probe", fn);
+    if (prec != QCD_F32 && prec != QCD_F64) return bad(QCD_EINVAL, "%s: unknown prec", fn);
+    if (reps < 1) return bad(QCD_EINVAL, "%s: reps < 1", fn);
+    QCD_TRY(check_ptr(scratch, fn));
+    if (scratch_bytes < probe_scratch_bytes(what)) return bad(QCD_EWORKSPACE, "%s: scratch smaller than qcd_probe_scratch_bytes", fn);
+    return launch_probe(what, prec, reps, scratch, (cudaStream_t)stream);
+}
+
 int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host, void *P_host,
                 void *device_work, void *stream) {
     const char *fn = "qcd_md_host";

@@ -107,6 +107,10 @@ int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, c
                          bool per_t, double *out, double *ws, cudaStream_t st);
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *lex, void *soa, bool unpack,
                 cudaStream_t st);
+// probes of the FMA / L1 / shared-memory / L2 rates (probe.cu)
+double probe_work(int what, int prec, int reps);
+size_t probe_scratch_bytes(int what);
+int launch_probe(int what, int prec, int reps, void *scratch, cudaStream_t st);
 int launch_get_map(const qcd_lattice *lat, int which, int32_t *out, cudaStream_t st);
 
 }  // namespace qcd

@@ -162,7 +162,7 @@ def test_mom_refresh_and_hot_start(qcd, orc_omp, prec, dims):
     U = lat.new_matrix_field(tdtype(prec))
     for sigma in (0.2, 0.5, 3.0):
         qcd.qcd_hot_start(lat, U, seed, sigma)
-        assert rel(host(qcd, lat, U), orc_omp.hot_start(dims, seed, sigma)) < tol * (10 if sigma > 1 else 1)
+        assert rel(host(qcd, lat, U), orc_omp.hot_start(dims, seed, sigma)) < tol
 
 
 # ------------------------------------------------------------------ plaquette, sums
@@ -192,8 +192,8 @@ def test_plaquette(qcd, orc_omp, prec, dims):
     qcd.qcd_plaquette(lat, dev(qcd, lat, G, prec), avg, per_t, ws)
     gavg, gper_t = orc_omp.plaquette(dims, G)
     scale = np.abs(gper_t).max()
-    assert np.abs(per_t.cpu().numpy() - gper_t).max() / scale < tol * 50  # sums of O(1) terms of both signs
-    assert abs(avg.item() - gavg) / scale < tol * 50
+    assert np.abs(per_t.cpu().numpy() - gper_t).max() / scale < tol
+    assert abs(avg.item() - gavg) / scale < tol
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -280,7 +280,7 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
     U = round_to(prec, inputs.random_matrix_field(17, lat.V) * 0.6)
     F = lat.new_matrix_field(tdtype(prec))
     qcd.qcd_gauge_force(lat, dev(qcd, lat, U, prec), F, 6.1)
-    assert rel(host(qcd, lat, F), orc.gauge_force(dims, 6.1, U)) < TOL[prec] * 5
+    assert rel(host(qcd, lat, F), orc.gauge_force(dims, 6.1, U)) < TOL[prec]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -376,7 +376,7 @@ def test_link_update_and_reunit(qcd, orc_omp, prec, dims):
         dU = dev(qcd, lat, U, prec)
         qcd.qcd_link_update(lat, dP, dU, big, reunit=False)
         ref = orc_omp.link_update(dims, big, P, U)
-        assert rel(host(qcd, lat, dU), ref) < TOL[prec] * max(1.0, big), big
+        assert rel(host(qcd, lat, dU), ref) < TOL[prec] * max(1.0, big / 20), big  # DESIGN.md R15: 2^n squarings amplify rounding by ~|eps P|
     # reunitarisation of links pushed off SU(3) by sigma = 1e-3 noise (config 3), GPU noise vs oracle noise
     dU = dev(qcd, lat, U, prec)
     qcd.qcd_perturb(lat, dU, seed + 1, 1e-3)
