@@ -63,6 +63,71 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
     return st;
 }
 
+// Lexicographic offsets of the periodic hops x -> x +- e_d for the direction d = (mu + k) & 3, k a compile-time
+// constant and mu the (rolled) loop variable.  Picking df[d] from a per-thread register array with a run-time d
+// compiles to branches, which keep the compiler from moving the next product's loads above the current one.  Two
+// ways around it, chosen by precision (measured at 32^3x64, profiles/r02_force_variants.md):
+//   ROT = true  (fp32: registers to spare, instruction issue is the limit)  the arrays are rotated at the end of
+//               every iteration so that entry k belongs to direction (mu + k) & 3: compile-time indices.
+//   ROT = false (fp64: every register counts)  the two possible hops per direction are block-uniform and sit in
+//               shared memory, tab[d] = stride_d, tab[4 + d] = -(L_d - 1) stride_d; a thread keeps eight wrap bits.
+template <bool ROT>
+struct Hops;
+
+template <>
+struct Hops<true> {
+    int df[4], db[4];
+    __device__ __forceinline__ void init(const LatP &lat, const Site &st, int *) {
+#pragma unroll
+        for (int d = 0; d < 4; d++) {
+            df[d] = dfwd(lat, st, d);
+            db[d] = dbwd(lat, st, d);
+        }
+    }
+    template <int K>
+    __device__ __forceinline__ int fwd(int) const { return df[K]; }
+    template <int K>
+    __device__ __forceinline__ int bwd(int) const { return db[K]; }
+    __device__ __forceinline__ void next() {
+        const int tf = df[0], tb = db[0];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            df[d] = df[d + 1];
+            db[d] = db[d + 1];
+        }
+        df[3] = tf;
+        db[3] = tb;
+    }
+};
+
+template <>
+struct Hops<false> {
+    const int *tab;  // shared, 8 ints
+    unsigned wrap;   // bit d: c[d] == L[d] - 1;  bit 4 + d: c[d] == 0
+    // every thread of the block calls init before the first use; the caller synchronises the block
+    __device__ __forceinline__ void init(const LatP &lat, const Site &st, int *t) {
+        if (threadIdx.x < 4) {
+            t[threadIdx.x] = lat.stride[threadIdx.x];
+            t[4 + threadIdx.x] = -(lat.L[threadIdx.x] - 1) * lat.stride[threadIdx.x];
+        }
+        tab = t;
+        wrap = 0;
+#pragma unroll
+        for (int d = 0; d < 4; d++) wrap |= (st.c[d] == lat.L[d] - 1 ? 1u << d : 0u) | (st.c[d] == 0 ? 16u << d : 0u);
+    }
+    template <int K>
+    __device__ __forceinline__ int fwd(int mu) const {
+        const int d = (mu + K) & 3;
+        return tab[d + 4 * ((wrap >> d) & 1u)];
+    }
+    template <int K>
+    __device__ __forceinline__ int bwd(int mu) const {
+        const int d = (mu + K) & 3;
+        return -tab[d + 4 * ((wrap >> (4 + d)) & 1u)];
+    }
+    __device__ __forceinline__ void next() {}
+};
+
 // Fixed-order sum of one double per thread over a block of ANY size (partial last warp included: no shuffle
 // reads a lane that was never launched).  Result valid in thread 0.  buf: NT doubles of shared memory.
 template <int NT>
@@ -248,14 +313,19 @@ struct Pend {
 // R13) and K = sum |P_ij|^2 of the updated momenta as by-products (PAPER.md:26 fused as in PAPER.md:32), one fp64
 // partial pair per block.
 template <typename T, bool FUSED, bool EARLYP, bool LINK, bool ANISO, bool SUMS, bool TMEM>
-__global__ void __launch_bounds__(FORCE_NT, 3)
+// resident blocks per SM: 3 in fp64 (168 registers), 4 in fp32 (128 registers) — measured best of 2..6
+__global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     force_plane_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */, const T eps,
                        const pair_t<T> *__restrict__ U, pair_t<T> *__restrict__ out, const T eps_u,
                        pair_t<T> *__restrict__ Uout, const T ws, const T wt, double *__restrict__ partial) {
     constexpr int TMEM_COLS = sizeof(T) == 8 ? 128 : 64;  // 4 x 18 (fp64) or 4 x 9 (fp32) words per thread
     __shared__ T pend_s[TMEM ? 1 : 4 * 9 * FORCE_NT];
     __shared__ uint32_t tmem_base;
+    __shared__ int hop_tab[8];
     Pend<T, TMEM> pend;
+    const Site st = tile_site(lat, tile, threadIdx.x);
+    Hops<sizeof(T) == 4> hop;
+    hop.init(lat, st, hop_tab);
     if (TMEM) {
         if (threadIdx.x < 32) tmem_alloc<TMEM_COLS>(&tmem_base);
         tmem_fence_before_sync();
@@ -263,27 +333,18 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
         tmem_fence_after_sync();
         pend.a = tmem_base + ((threadIdx.x & ~31u) << 16);
     } else {
+        __syncthreads();
         pend.p = pend_s + threadIdx.x;
     }
     double sumW = 0.0, sumK = 0.0;
-    const Site st = tile_site(lat, tile, threadIdx.x);
     const int V = lat.V;
     const int par = st.par;
     const int cb = cb_of(lat, st.s, par);
-    int df[4], db[4];
-#pragma unroll
-    for (int d = 0; d < 4; d++) {
-        df[d] = dfwd(lat, st, d);
-        db[d] = dbwd(lat, st, d);
-    }
     pend.zero();
 
-    // df[k], db[k] are rotated at the end of every iteration so that they belong to direction (mu + k) & 3: the
-    // neighbour offsets are then picked with compile-time indices (run-time selects compile to branches, which
-    // keep the compiler from moving the next product's loads above the current one)
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
-        const int dfm = df[0];
+        const int dfm = hop.template fwd<0>(mu);
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
         M3<T> Pm;
         if (FUSED && EARLYP) load_link_cs(Pm, out, V, mu, cb);
@@ -294,7 +355,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
             const int nu = mu + k;
             const T w = ANISO ? (nu == 3 ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;
-            const int cb_pn = cb_of(lat, st.s + df[k], par ^ 1);  // x + nu
+            const int cb_pn = cb_of(lat, st.s + (k == 1 ? hop.template fwd<1>(mu) : k == 2 ? hop.template fwd<2>(mu) : hop.template fwd<3>(mu)), par ^ 1);  // x + nu
             M3<T> X, Y, Z;
             load_link(X, U, V, nu, cb_pm);
             load_link(Y, U, V, mu, cb_pn);
@@ -317,7 +378,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
             const int nu = (mu + k) & 3;
             const T w = ANISO ? ((mu == 3 || nu == 3) ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;  // warp-uniform
-            const int dbn = db[k];
+            const int dbn = k == 1 ? hop.template bwd<1>(mu) : k == 2 ? hop.template bwd<2>(mu) : hop.template bwd<3>(mu);
             const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
             const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
             M3<T> X, Y, Z;
@@ -332,18 +393,16 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
         M3<T> Um, F;
         load_link(Um, U, V, mu, cb);
         TA<T> acc;
-        pend.load(mu, acc);
-        mul_ta<true, false>(acc, Um, A);
+        mul_ta<false, false>(acc, Um, A);
+        {  // the parts that waited in Tensor Memory join after the product: their load is off the critical path
+            TA<T> w;
+            pend.load(mu, w);
+#pragma unroll
+            for (int j = 0; j < 9; j++) acc.v[j] += w.v[j];
+        }
         force_from_ta(F, acc, c);
         finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
-        const int tf = df[0], tb = db[0];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            df[d] = df[d + 1];
-            db[d] = db[d + 1];
-        }
-        df[3] = tf;
-        db[3] = tb;
+        hop.next();
     }
     if (TMEM) {
         tmem_wait_st();
@@ -368,24 +427,19 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
     force_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */, const T eps,
                  const pair_t<T> *__restrict__ U, pair_t<T> *__restrict__ out, const T eps_u,
                  pair_t<T> *__restrict__ Uout, const T ws, const T wt, double *__restrict__ partial) {
+    __shared__ int hop_tab[8];
     double sumW = 0.0, sumK = 0.0;
     const Site st = tile_site(lat, tile, threadIdx.x);
+    Hops<sizeof(T) == 4> hop;
+    hop.init(lat, st, hop_tab);
+    __syncthreads();
     const int V = lat.V;
     const int par = st.par;
     const int cb = cb_of(lat, st.s, par);
-    int df[4], db[4];
-#pragma unroll
-    for (int d = 0; d < 4; d++) {
-        df[d] = dfwd(lat, st, d);
-        db[d] = dbwd(lat, st, d);
-    }
 
-    // df[k], db[k] are rotated at the end of every iteration so that they belong to direction (mu + k) & 3: the
-    // neighbour offsets are then picked with compile-time indices (run-time selects compile to branches, which
-    // keep the compiler from moving the next staple's loads above the current product)
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
-        const int dfm = df[0];
+        const int dfm = hop.template fwd<0>(mu);
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
         M3<T> A, Pm;
         // the momenta come straight from HBM (no reuse): with registers to spare (fp32) their loads are issued
@@ -397,7 +451,8 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
             const int nu = (mu + k) & 3;
             const T w = ANISO ? ((mu == 3 || nu == 3) ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;  // warp-uniform
-            const int dfn = df[k], dbn = db[k];
+            const int dfn = k == 1 ? hop.template fwd<1>(mu) : k == 2 ? hop.template fwd<2>(mu) : hop.template fwd<3>(mu);
+            const int dbn = k == 1 ? hop.template bwd<1>(mu) : k == 2 ? hop.template bwd<2>(mu) : hop.template bwd<3>(mu);
             const int cb_pn = cb_of(lat, st.s + dfn, par ^ 1);      // x + nu
             const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
             const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
@@ -425,14 +480,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
         project_force(F, W, c);
         if (SUMS) sumW += (double)W.re[0] + (double)W.re[4] + (double)W.re[8];
         finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
-        const int tf = df[0], tb = db[0];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            df[d] = df[d + 1];
-            db[d] = db[d + 1];
-        }
-        df[3] = tf;
-        db[3] = tb;
+        hop.next();
     }
     if (SUMS) {
         __shared__ double red[FORCE_NT];
