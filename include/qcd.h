@@ -306,6 +306,39 @@ int qcd_perturb(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, v
 int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, const uint32_t *site,
                    const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, void *stream);
 
+/* ---- domain decomposition in t with a one-site halo ("multi-GPU (parallel
+ * architecture) support"; PAPER.md:121 overlapping communication and computation "is work in progress").
+ * A SLAB lattice holds t_count consecutive global timeslices starting at t_begin plus one halo timeslice on either
+ * side: local extents (Lx, Ly, Lz, t_count + 2); local timeslice te is the global timeslice (t_begin + te - 1) mod Lt,
+ * te = 0 and te = t_count + 1 are the halos.  Fields on a slab lattice have the usual device layout for the local
+ * extents.  Semantics of every call on a slab lattice:
+ *   - the stencil calls (qcd_gauge_force*, qcd_force_mom_update*, qcd_md_step*, qcd_leapfrog*) update the INTERIOR
+ *     timeslices only and read the halos, which the caller refreshes with qcd_copy_timeslices after every link
+ *     update (one exchange per force evaluation: from the lower neighbour's last interior timeslice into te = 0,
+ *     all four links; from the upper neighbour's first interior timeslice into te = t_count + 1, mu_mask 0x7);
+ *   - the site-local calls act on all stored timeslices (halo values are recomputed or overwritten by the next
+ *     exchange); EVEN / ODD always mean the GLOBAL parity;
+ *   - the generator is keyed on the GLOBAL lexicographic site: qcd_mom_refresh, qcd_hot_start, qcd_perturb and
+ *     qcd_spinor_gaussian give, timeslice by timeslice, exactly the field of the undecomposed lattice (halos
+ *     included, so no exchange is needed after them);
+ *   - qcd_force_mom_update_sums averages the plaquette over the interior sites and sums K over them; the
+ *     reductions with per-timeslice outputs (qcd_plaquette out_per_t, qcd_sum_multi, qcd_inner_product_multi)
+ *     return t_count + 2 values of which the interior ones are the global lattice's; ranks are combined in fixed
+ *     rank order by the caller (paper_1212_0785_b200/slabs.py).  qcd_trajectory and the by-product per-timeslice
+ *     sums need the whole lattice.
+ * qcd_copy_timeslices is the transport: it copies nt timeslices of a pair-layout field (ncomp reals per site, 72 for
+ * matrix fields; mu_mask selects the links of a matrix field, bit mu) between two lattices with the same spatial
+ * extents; dst may be a peer GPU's memory (direct stores over NVLink).  QCD_EDIMS if the spatial extents differ. */
+int qcd_lattice_create_slab(const int global_dims[4], int t_begin, int t_count, qcd_lattice **out);
+/* A second descriptor of the same stored lattice (same extents, layout, generator offsets) whose stencil calls
+ * update the timeslices [t0, t1) only: the boundary / interior split that lets the force of the inner timeslices
+ * run while the halos travel.  Destroy it with qcd_lattice_destroy. */
+int qcd_lattice_view_t(const qcd_lattice *lat, int t0, int t1, qcd_lattice **out);
+/* local (stored) extents and the interior timeslice range [interior_t[0], interior_t[1]) (NULL: not wanted) */
+int qcd_lattice_dims(const qcd_lattice *lat, int dims[4], int interior_t[2]);
+int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
+                        int dst_t, int nt, int prec, int ncomp, unsigned mu_mask, void *stream);
+
 /* ---- measured denominators ("Measure DFMA/FFMA peaks with a probe") --------------------
  * One kernel launch per probe, enqueued on `stream` like every other call and timed by the caller with CUDA
  * events (bench.py --peaks): rate = qcd_probe_work(...) / elapsed.

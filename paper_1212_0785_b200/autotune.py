@@ -30,8 +30,9 @@ def _divisors(n, even=False):
 
 
 def force_tiles(dims, limit_sites, keep=12):
-    """4-D tiles that divide the lattice, fill the block (the largest site count <= limit) and have the longest x
-    rows first (coalescing), then the smallest surface"""
+    """4-D tiles that divide the lattice and fill the block — the largest site count <= limit, and the next
+    smaller one when it allows whole x rows (48-wide lattices: 96-site tiles of whole rows against 128-site tiles
+    of 16-wide rows) — longest x rows first (coalescing), then the smallest surface"""
     cands = []
     for t in itertools.product(_divisors(dims[0], True), _divisors(dims[1]), _divisors(dims[2]), _divisors(dims[3])):
         sites = t[0] * t[1] * t[2] * t[3]
@@ -42,7 +43,9 @@ def force_tiles(dims, limit_sites, keep=12):
     top = max(s for s, _ in cands)
     full = [t for s, t in cands if s == top]
     full.sort(key=lambda t: (-min(t[0], 32), sum(1.0 / x for x in t)))
-    return full[:keep]
+    rows = [t for s, t in cands if t[0] == dims[0] and s >= 0.75 * top and s != top]
+    rows.sort(key=lambda t: (-t[0] * t[1] * t[2] * t[3], sum(1.0 / x for x in t)))
+    return full[:keep] + rows[:4]
 
 
 def _time(fn, warm=3, reps=10):

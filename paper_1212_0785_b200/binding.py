@@ -26,6 +26,10 @@ MAP_CB_OF_LEX, MAP_LEX_OF_CB, MAP_NBR_FWD0, MAP_NBR_BWD0, MAP_PARITY, MAP_TSLICE
 _vp, _i, _d, _u64, _u32, _sz = C.c_void_p, C.c_int, C.c_double, C.c_uint64, C.c_uint32, C.c_size_t
 SIGNATURES = {
     "qcd_lattice_create": (_i, [C.POINTER(C.c_int * 4), C.POINTER(_vp)]),
+    "qcd_lattice_create_slab": (_i, [C.POINTER(C.c_int * 4), _i, _i, C.POINTER(_vp)]),
+    "qcd_lattice_view_t": (_i, [_vp, _i, _i, C.POINTER(_vp)]),
+    "qcd_lattice_dims": (_i, [_vp, C.POINTER(C.c_int * 4), C.POINTER(C.c_int * 2)]),
+    "qcd_copy_timeslices": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, _i, _i, C.c_uint, _vp]),
     "qcd_lattice_destroy": (_i, [_vp]),
     "qcd_lattice_volume": (C.c_int64, [_vp]),
     "qcd_field_bytes": (_sz, [_vp, _i, _i]),
@@ -121,15 +125,34 @@ def _stream(stream):
 class Lattice:
     """qcd_lattice handle (host side)."""
 
-    def __init__(self, dims):
-        self.dims = tuple(int(d) for d in dims)
+    def __init__(self, dims, slab=None):
+        """dims: extents of the (global) lattice; slab = (t_begin, t_count): the slab lattice of
+        qcd_lattice_create_slab (stored extents (Lx, Ly, Lz, t_count + 2), interior timeslices 1 .. t_count)"""
+        gdims = tuple(int(d) for d in dims)
         h = _vp()
-        arr = (C.c_int * 4)(*self.dims) if len(self.dims) == 4 else None
+        arr = (C.c_int * 4)(*gdims) if len(gdims) == 4 else None
         if arr is None:
             raise QcdError(EINVAL, "dims must have 4 entries")
-        _check(lib.qcd_lattice_create(C.byref(arr), C.byref(h)))
+        if slab is None:
+            _check(lib.qcd_lattice_create(C.byref(arr), C.byref(h)))
+        else:
+            _check(lib.qcd_lattice_create_slab(C.byref(arr), int(slab[0]), int(slab[1]), C.byref(h)))
         self.handle = h
         self.V = int(lib.qcd_lattice_volume(h))
+        d, it = (C.c_int * 4)(), (C.c_int * 2)()
+        _check(lib.qcd_lattice_dims(h, C.byref(d), C.byref(it)))
+        self.dims = tuple(d)          # stored (local) extents
+        self.interior_t = tuple(it)   # timeslices the stencil kernels update
+        self.global_dims, self.slab = gdims, slab
+
+    def view_t(self, t0, t1):
+        """the same stored lattice with the stencil calls restricted to the timeslices [t0, t1) (qcd_lattice_view_t)"""
+        v = object.__new__(Lattice)
+        h = _vp()
+        _check(lib.qcd_lattice_view_t(self.handle, int(t0), int(t1), C.byref(h)))
+        v.handle, v.V, v.dims, v.interior_t = h, self.V, self.dims, (int(t0), int(t1))
+        v.global_dims, v.slab = self.global_dims, self.slab
+        return v
 
     def __del__(self):
         h = getattr(self, "handle", None)
@@ -333,6 +356,11 @@ def qcd_md_host(lat, U_host, P_host, beta, eps, nsteps, device_work, stream=None
     """U_host, P_host: host tensors (pinned for asynchronous copies) in the canonical layout [V,4,3,3,2]."""
     _check(lib.qcd_md_host(lat.handle, _prec(U_host), beta, eps, nsteps, _ptr(U_host), _ptr(P_host),
                            _ptr(device_work), _stream(stream)))
+
+
+def qcd_copy_timeslices(src_lat, src, src_t, dst_lat, dst, dst_t, nt, ncomp=72, mu_mask=0xF, stream=None):
+    _check(lib.qcd_copy_timeslices(src_lat.handle, _ptr(src), src_t, dst_lat.handle, _ptr(dst), dst_t, nt, _prec(src),
+                                   ncomp, mu_mask, _stream(stream)))
 
 
 def qcd_probe_launch(what, prec, reps, scratch, stream=None):

@@ -42,6 +42,11 @@ static int check_subset(int subset, const char *fn) {
     if (subset != QCD_ALL && subset != QCD_EVEN && subset != QCD_ODD) return bad(QCD_EINVAL, "%s: unknown subset", fn);
     return QCD_OK;
 }
+// EVEN / ODD always mean the GLOBAL parity; a slab lattice whose first stored timeslice is globally odd flips them
+static int local_subset(const qcd_lattice *lat, int subset) {
+    if (subset == QCD_ALL || !lat->par_flip) return subset;
+    return subset == QCD_EVEN ? QCD_ODD : QCD_EVEN;
+}
 static int check_ptr(const void *p, const char *fn) {
     if (!p) return bad(QCD_EINVAL, "%s: NULL field pointer", fn);
     if (((uintptr_t)p) & 15) return bad(QCD_EALIGN, "%s: field pointer not 16-byte aligned", fn);
@@ -73,17 +78,18 @@ using namespace qcd;
 
 extern "C" {
 
-int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
-    if (!dims || !out) return bad(QCD_EINVAL, "%s: NULL argument", "qcd_lattice_create");
+// the descriptor of a lattice with extents dims whose stencil kernels update the timeslices [t0, t1)
+static int make_lattice(const int dims[4], int t0, int t1, long long site_off, long long gV, int par_flip,
+                        qcd_lattice **out, const char *fn) {
     long long V = 1;
     for (int d = 0; d < 4; d++) {
-        if (dims[d] < 2 || (dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", "qcd_lattice_create");
+        if (dims[d] < 2 || (dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", fn);
         V *= dims[d];
         // 36 V < 2^32: the kernels index the 36 V complex pairs of a matrix field with 32 bits
-        if (36 * (V + 32) >= (1ll << 32)) return bad(QCD_EDIMS, "%s: V must be < 2^32 / 36", "qcd_lattice_create");
+        if (36 * (V + 32) >= (1ll << 32)) return bad(QCD_EDIMS, "%s: V must be < 2^32 / 36", fn);
     }
     qcd_lattice *lat = new (std::nothrow) qcd_lattice;
-    if (!lat) return bad(QCD_EINVAL, "%s: out of host memory", "qcd_lattice_create");
+    if (!lat) return bad(QCD_EINVAL, "%s: out of host memory", fn);
     int stride = 1;
     for (int d = 0; d < 4; d++) {
         lat->p.L[d] = dims[d];
@@ -92,6 +98,11 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
     }
     lat->p.V = (int)V;
     lat->p.Vh = (int)(V / 2);
+    lat->p.t0 = t0;
+    lat->p.t1 = t1;
+    lat->p.site_off = (int)site_off;
+    lat->p.gV = (int)(gV ? gV : V);
+    lat->par_flip = par_flip;
     const int Vsh = lat->p.Vh / dims[3];
     lat->red_chunks_per_seg = (Vsh + RED_CHUNK - 1) / RED_CHUNK;
     lat->red_nseg = 2 * dims[3];
@@ -102,6 +113,52 @@ int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
     default_force_tile(lat->p, 2, lat->tile_all);
     default_force_tile(lat->p, 1, lat->tile_par);
     *out = lat;
+    return QCD_OK;
+}
+
+int qcd_lattice_create(const int dims[4], qcd_lattice **out) {
+    if (!dims || !out) return bad(QCD_EINVAL, "%s: NULL argument", "qcd_lattice_create");
+    return make_lattice(dims, 0, dims[3], 0, 0, 0, out, "qcd_lattice_create");
+}
+
+int qcd_lattice_create_slab(const int global_dims[4], int t_begin, int t_count, qcd_lattice **out) {
+    const char *fn = "qcd_lattice_create_slab";
+    if (!global_dims || !out) return bad(QCD_EINVAL, "%s: NULL argument", fn);
+    long long gV = 1;
+    for (int d = 0; d < 4; d++) {
+        if (global_dims[d] < 2 || (global_dims[d] & 1)) return bad(QCD_EDIMS, "%s: extents must be even and >= 2", fn);
+        gV *= global_dims[d];
+    }
+    const int Lt = global_dims[3];
+    if (t_count < 2 || (t_count & 1) || t_count > Lt || t_begin < 0 || t_begin >= Lt)
+        return bad(QCD_EDIMS, "%s: t_count must be even, 2..Lt, and 0 <= t_begin < Lt", fn);
+    const int dims[4] = {global_dims[0], global_dims[1], global_dims[2], t_count + 2};
+    const long long Vs = gV / Lt;
+    // slab timeslice te is global timeslice (t_begin + te - 1) mod Lt
+    return make_lattice(dims, 1, t_count + 1, Vs * ((t_begin - 1 + Lt) % Lt), gV, (t_begin - 1 + Lt) & 1, out, fn);
+}
+
+int qcd_lattice_view_t(const qcd_lattice *lat, int t0, int t1, qcd_lattice **out) {
+    const char *fn = "qcd_lattice_view_t";
+    if (!lat || !out) return bad(QCD_EINVAL, "%s: NULL argument", fn);
+    if (t0 < 0 || t1 > lat->p.L[3] || t1 <= t0) return bad(QCD_EDIMS, "%s: need 0 <= t0 < t1 <= Lt", fn);
+    qcd_lattice *v = new (std::nothrow) qcd_lattice(*lat);
+    if (!v) return bad(QCD_EINVAL, "%s: out of host memory", fn);
+    v->p.t0 = t0;
+    v->p.t1 = t1;
+    default_force_tile(v->p, 2, v->tile_all);
+    default_force_tile(v->p, 1, v->tile_par);
+    *out = v;
+    return QCD_OK;
+}
+
+int qcd_lattice_dims(const qcd_lattice *lat, int dims[4], int interior_t[2]) {
+    if (!lat || !dims) return bad(QCD_EINVAL, "%s: NULL argument", "qcd_lattice_dims");
+    for (int d = 0; d < 4; d++) dims[d] = lat->p.L[d];
+    if (interior_t) {
+        interior_t[0] = lat->p.t0;
+        interior_t[1] = lat->p.t1;
+    }
     return QCD_OK;
 }
 
@@ -133,7 +190,7 @@ int qcd_gauge_force(const qcd_lattice *lat, int prec, int subset, double beta, c
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(F, fn));
     QCD_TRY(check_alias(U, F, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_gauge_force(lat, prec, subset, beta, 0.0, U, F, false, (cudaStream_t)stream);
+    return launch_gauge_force(lat, prec, local_subset(lat, subset), beta, 0.0, U, F, false, (cudaStream_t)stream);
 }
 
 int qcd_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P, void *stream) {
@@ -143,7 +200,7 @@ int qcd_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, con
     QCD_TRY(check_ptr(F, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(F, P, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_mom_update(lat, prec, subset, eps, F, P, (cudaStream_t)stream);
+    return launch_mom_update(lat, prec, local_subset(lat, subset), eps, F, P, (cudaStream_t)stream);
 }
 
 int qcd_force_mom_update(const qcd_lattice *lat, int prec, int subset, double beta, double eps, const void *U,
@@ -154,7 +211,7 @@ int qcd_force_mom_update(const qcd_lattice *lat, int prec, int subset, double be
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_gauge_force(lat, prec, subset, beta, eps, U, P, true, (cudaStream_t)stream);
+    return launch_gauge_force(lat, prec, local_subset(lat, subset), beta, eps, U, P, true, (cudaStream_t)stream);
 }
 
 int qcd_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U, int reunit,
@@ -165,7 +222,7 @@ int qcd_link_update(const qcd_lattice *lat, int prec, int subset, double eps, co
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_alias(P, U, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_link_update(lat, prec, subset, eps, P, U, reunit ? 1 : 0, (cudaStream_t)stream);
+    return launch_link_update(lat, prec, local_subset(lat, subset), eps, P, U, reunit ? 1 : 0, (cudaStream_t)stream);
 }
 
 int qcd_reunit(const qcd_lattice *lat, int prec, int subset, void *U, void *stream) {
@@ -173,7 +230,7 @@ int qcd_reunit(const qcd_lattice *lat, int prec, int subset, void *U, void *stre
     QCD_TRY(check_common(lat, prec, fn));
     QCD_TRY(check_subset(subset, fn));
     QCD_TRY(check_ptr(U, fn));
-    return launch_link_update(lat, prec, subset, 0.0, U, U, 2, (cudaStream_t)stream);
+    return launch_link_update(lat, prec, local_subset(lat, subset), 0.0, U, U, 2, (cudaStream_t)stream);
 }
 
 int qcd_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *P,
@@ -182,7 +239,7 @@ int qcd_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed,
     QCD_TRY(check_common(lat, prec, fn));
     QCD_TRY(check_subset(subset, fn));
     QCD_TRY(check_ptr(P, fn));
-    return launch_mom_refresh(lat, prec, subset, seed, stream_id, P, (cudaStream_t)stream);
+    return launch_mom_refresh(lat, prec, local_subset(lat, subset), seed, stream_id, P, (cudaStream_t)stream);
 }
 
 int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
@@ -213,7 +270,7 @@ int qcd_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, c
     QCD_TRY(check_units(lat, kind == QCD_SUM_SCALAR ? ncomp : ncomp / 2, fn));
     QCD_TRY(check_ptr(field, fn));
     if (!out || !workspace) return bad(QCD_EINVAL, "%s: NULL output or workspace", fn);
-    return launch_sum(lat, prec, subset, kind, ncomp, field, out, (double *)workspace, (cudaStream_t)stream);
+    return launch_sum(lat, prec, local_subset(lat, subset), kind, ncomp, field, out, (double *)workspace, (cudaStream_t)stream);
 }
 
 int qcd_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field, const int32_t *subset_id,
@@ -392,7 +449,7 @@ int qcd_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, double b
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(F, fn));
     QCD_TRY(check_alias(U, F, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_gauge_force_aniso(lat, prec, subset, beta_s, beta_t, 0.0, U, F, false, (cudaStream_t)stream);
+    return launch_gauge_force_aniso(lat, prec, local_subset(lat, subset), beta_s, beta_t, 0.0, U, F, false, (cudaStream_t)stream);
 }
 
 int qcd_force_mom_update_aniso(const qcd_lattice *lat, int prec, int subset, double beta_s, double beta_t,
@@ -403,7 +460,7 @@ int qcd_force_mom_update_aniso(const qcd_lattice *lat, int prec, int subset, dou
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
-    return launch_gauge_force_aniso(lat, prec, subset, beta_s, beta_t, eps, U, P, true, (cudaStream_t)stream);
+    return launch_gauge_force_aniso(lat, prec, local_subset(lat, subset), beta_s, beta_t, eps, U, P, true, (cudaStream_t)stream);
 }
 
 int qcd_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
@@ -450,7 +507,7 @@ int qcd_spinor_gaussian(const qcd_lattice *lat, int prec, int subset, uint64_t s
     QCD_TRY(check_common(lat, prec, fn));
     QCD_TRY(check_subset(subset, fn));
     QCD_TRY(check_ptr(eta, fn));
-    return launch_spinor_gaussian(lat, prec, subset, seed, stream_id, eta, (cudaStream_t)stream);
+    return launch_spinor_gaussian(lat, prec, local_subset(lat, subset), seed, stream_id, eta, (cudaStream_t)stream);
 }
 
 static int check_inner(const qcd_lattice *lat, int prec, int nc, const void *a, const void *b, const double *out,
@@ -469,7 +526,7 @@ int qcd_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, cons
     const char *fn = "qcd_inner_product";
     QCD_TRY(check_inner(lat, prec, nc, a, b, out, workspace, fn));
     QCD_TRY(check_subset(subset, fn));
-    return launch_inner_product(lat, prec, subset, nc, a, b, false, out, (double *)workspace, (cudaStream_t)stream);
+    return launch_inner_product(lat, prec, local_subset(lat, subset), nc, a, b, false, out, (double *)workspace, (cudaStream_t)stream);
 }
 
 int qcd_inner_product_multi(const qcd_lattice *lat, int prec, int nc, const void *a, const void *b, double *out,
@@ -491,7 +548,8 @@ int qcd_tune_set(const qcd_lattice *lat, int prec, int subset, int kernel, int v
         if (tile && tile[0]) {
             long sites = 1;
             for (int d = 0; d < 4; d++) {
-                if (tile[d] < 1 || lat->p.L[d] % tile[d]) return bad(QCD_EINVAL, "%s: tile must divide the lattice", fn);
+                const int ext = d == 3 ? lat->p.t1 - lat->p.t0 : lat->p.L[d];
+                if (tile[d] < 1 || ext % tile[d]) return bad(QCD_EINVAL, "%s: tile must divide the lattice", fn);
                 sites *= tile[d];
                 cfg.tile[d] = tile[d];
             }
@@ -581,6 +639,23 @@ int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, c
     const char *fn = "qcd_rng_blocks";
     if (n < 0 || (n > 0 && (!site || !mu_j))) return bad(QCD_EINVAL, "%s: bad arguments", fn);
     return launch_rng_blocks(seed, stream_id, purpose, n, site, mu_j, words, uniforms, gauss, (cudaStream_t)stream);
+}
+
+int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
+                        int dst_t, int nt, int prec, int ncomp, unsigned mu_mask, void *stream) {
+    const char *fn = "qcd_copy_timeslices";
+    QCD_TRY(check_common(src_lat, prec, fn));
+    QCD_TRY(check_common(dst_lat, prec, fn));
+    QCD_TRY(check_ptr(src, fn));
+    QCD_TRY(check_ptr(dst, fn));
+    for (int d = 0; d < 3; d++)
+        if (src_lat->p.L[d] != dst_lat->p.L[d]) return bad(QCD_EDIMS, "%s: the two lattices differ in a spatial extent", fn);
+    if (ncomp < 2 || (ncomp & 1)) return bad(QCD_EINVAL, "%s: ncomp must be even (pair layout)", fn);
+    if (nt < 1 || src_t < 0 || src_t + nt > src_lat->p.L[3] || dst_t < 0 || dst_t + nt > dst_lat->p.L[3])
+        return bad(QCD_EINVAL, "%s: timeslice range outside a lattice", fn);
+    if (src == dst && src_t < dst_t + nt && dst_t < src_t + nt) return bad(QCD_EALIAS, "%s: overlapping timeslices of one field", fn);
+    return launch_copy_timeslices(src_lat, src, src_t, dst_lat, dst, dst_t, nt, prec, ncomp / 2, mu_mask,
+                                  (cudaStream_t)stream);
 }
 
 size_t qcd_probe_scratch_bytes(int what) {

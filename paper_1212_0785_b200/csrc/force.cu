@@ -57,7 +57,7 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
     st.par = par;
     st.c[1] = by * tile.T[1] + jy;
     st.c[2] = bz * tile.T[2] + jz;
-    st.c[3] = bt * tile.T[3] + jt;
+    st.c[3] = lat.t0 + bt * tile.T[3] + jt;  // the interior timeslices [t0, t1) of a slab lattice; t0 = 0 otherwise
     st.c[0] = bx * tile.T[0] + 2 * jx + ((st.c[1] + st.c[2] + st.c[3] + par) & 1);
     st.s = st.c[0] + lat.L[0] * (st.c[1] + lat.L[1] * (st.c[2] + lat.L[2] * st.c[3]));
     return st;
@@ -508,7 +508,7 @@ static void tile_from_extents(const LatP &lat, int subset, const int t[4], TileP
     tp.par0 = subset == QCD_ODD ? 1 : 0;
     for (int d = 0; d < 4; d++) {
         tp.T[d] = t[d];
-        tp.nt[d] = lat.L[d] / t[d];
+        tp.nt[d] = (d == 3 ? lat.t1 - lat.t0 : lat.L[d]) / t[d];
     }
     tp.tsp = (tp.T[0] / 2) * tp.T[1] * tp.T[2] * tp.T[3];
 }
@@ -519,7 +519,7 @@ static void tile_from_extents(const LatP &lat, int subset, const int t[4], TileP
 void default_force_tile(const LatP &lat, int npar, int out[4]) {
     int best[4] = {2, 1, 1, 1};
     int dv[4][128], nd[4];
-    for (int d = 0; d < 4; d++) nd[d] = divisors(lat.L[d], d == 0, dv[d]);
+    for (int d = 0; d < 4; d++) nd[d] = divisors(d == 3 ? lat.t1 - lat.t0 : lat.L[d], d == 0, dv[d]);
     double best_score = -1e300;
     for (int a = 0; a < nd[0]; a++)
         for (int b = 0; b < nd[1]; b++)
@@ -532,8 +532,12 @@ void default_force_tile(const LatP &lat, int npar, int out[4]) {
                     double surf = 0;
                     for (int k = 0; k < 4; k++) surf += vol / t[k];
                     // more threads first; then x extent up to 32 (256-byte rows per parity in fp64; measured best on
-                    // B200); then compactness
-                    const double score = threads * 1e6 + (t[0] >= 32 ? 32 : t[0]) * 1e3 - surf / vol * 100.0;
+                    // B200); then compactness; among equals the extent goes to y before z before t: consecutive
+                    // threads of a warp are then consecutive in memory (the site index runs x, y, z, t), and a tile
+                    // inside one timeslice gives per-timeslice sums as a by-product (32x2x2x1 beats 32x1x2x2 by 3.5 %
+                    // at 32^3x64, profiles/r02_tiles.md)
+                    const double score = threads * 1e6 + (t[0] >= 32 ? 32 : t[0]) * 1e3 - surf / vol * 100.0 +
+                                         t[1] * 1e-2 + t[2] * 1e-4;
                     if (score > best_score) {
                         best_score = score;
                         memcpy(best, t, sizeof best);
@@ -646,7 +650,8 @@ static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, doubl
         return QCD_EWORKSPACE;
     }
     const bool plane = fs.variant != QCD_FORCE_STAPLE;
-    if (out_per_t && !(plane && fs.tp.T[3] == 1)) return -1;
+    const bool slab = lat->p.t0 != 0 || lat->p.t1 != lat->p.L[3];
+    if (out_per_t && !(plane && fs.tp.T[3] == 1 && !slab)) return -1;
     const T c = (T)(beta / 12.0);
     if (Uout)
         launch_force_k<T, true, true, false, true>(lat, fs, c, (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u,
@@ -656,7 +661,8 @@ static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, doubl
                                                     nullptr, T(0), T(0), ws, st);
     QCD_TRY_RC(check_launch("force sums"));
     // plane kernel: sum of the six plaquette traces per site; staple kernel: sum_mu Re tr W_mu = 4 x that
-    const double V = (double)lat->p.V;
+    // a slab lattice sums (and averages) over its interior timeslices only
+    const double V = (double)(lat->p.V / lat->p.L[3]) * (double)(lat->p.t1 - lat->p.t0);
     QCD_TRY_RC(launch_sum_partials(ws, 1, blocks, 1.0 / ((plane ? 18.0 : 72.0) * V), out_plaq, st));
     if (out_per_t) {  // blocks of one timeslice are consecutive (the t index of the tile is the slowest)
         const int Lt = lat->p.L[3];

@@ -28,19 +28,22 @@ __global__ void __launch_bounds__(256) pack_kernel(const LatP lat, const int nco
 // odd site because Lx is even).  Site stride in shared memory is ncomp+2 reals (bank spread).
 constexpr int PK_SITES = 64;
 
+// site0, site_end: the lexicographic range handled (whole lattice, or whole timeslices of it); the canonical array
+// starts at site0.
 template <typename T, bool UNPACK>
 __global__ void __launch_bounds__(256) pack_tr_kernel(const LatP lat, const int ncomp, const bool matrix,
-                                                      const T *__restrict__ src, T *__restrict__ dst) {
+                                                      const T *__restrict__ src, T *__restrict__ dst,
+                                                      const int site0, const int site_end) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *sm = reinterpret_cast<T *>(smem_raw);
     const int ss = ncomp + 2;
-    const int s0 = blockIdx.x * PK_SITES;
-    const int ns = min(PK_SITES, lat.V - s0);  // V is even and s0 is even: ns is even
+    const int s0 = site0 + blockIdx.x * PK_SITES;
+    const int ns = min(PK_SITES, site_end - s0);  // the range and s0 are even: ns is even
     const int nh = ns >> 1;
     const int h0 = s0 >> 1;
     const int nel = ns * ncomp;
-    const T *aos_in = UNPACK ? nullptr : src + (size_t)s0 * ncomp;
-    T *aos_out = UNPACK ? dst + (size_t)s0 * ncomp : nullptr;
+    const T *aos_in = UNPACK ? nullptr : src + (size_t)(s0 - site0) * ncomp;
+    T *aos_out = UNPACK ? dst + (size_t)(s0 - site0) * ncomp : nullptr;
     if (!UNPACK)
         for (int i = threadIdx.x; i < nel; i += blockDim.x) sm[(i / ncomp) * ss + i % ncomp] = aos_in[i];
     else {
@@ -98,22 +101,72 @@ __global__ void map_kernel(const LatP lat, const int which, int32_t *__restrict_
     else out[s] = st.c[3];
 }
 
+// the transposing kernel on the lexicographic range [site0, site_end) (both even)
+static int launch_pack_range(const qcd_lattice *lat, int prec, int ncomp, bool matrix, const void *src, void *dst,
+                             bool unpack, int site0, int site_end, cudaStream_t st) {
+    const size_t rb = prec == QCD_F64 ? 8 : 4;
+    const size_t shm = (size_t)PK_SITES * (ncomp + 2) * rb;
+    const int blocks = (site_end - site0 + PK_SITES - 1) / PK_SITES;
+    if (prec == QCD_F64) {
+        if (unpack) pack_tr_kernel<double, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst, site0, site_end);
+        else pack_tr_kernel<double, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst, site0, site_end);
+    } else {
+        if (unpack) pack_tr_kernel<float, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst, site0, site_end);
+        else pack_tr_kernel<float, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst, site0, site_end);
+    }
+    return check_launch(unpack ? "unpack" : "pack");
+}
+
+int launch_pack_slab(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *src, void *dst, bool unpack,
+                     int t_begin, int nt, cudaStream_t st) {
+    const int Vs = lat->p.V / lat->p.L[3];
+    return launch_pack_range(lat, prec, ncomp, pairs, src, dst, unpack, t_begin * Vs, (t_begin + nt) * Vs, st);
+}
+
+// One thread per site of the `nt` source timeslices: copies the units of the links selected by mu_mask (matrix
+// fields) or all nc units from the source field to the same spatial site of the destination timeslices.  The two
+// lattices share the spatial extents; each side is addressed with its own checkerboard index (the parity of a site
+// depends on its local t).  With a peer pointer as dst this kernel is the NVLink transport of the halo exchange.
+template <typename T>
+__global__ void __launch_bounds__(256) copy_timeslices_kernel(const LatP src_lat, const pair_t<T> *__restrict__ src,
+                                                              const int src_t, const LatP dst_lat,
+                                                              pair_t<T> *__restrict__ dst, const int dst_t, const int nt,
+                                                              const int nc, const unsigned mu_mask) {
+    const int Vsh = src_lat.Vh / src_lat.L[3];  // sites per parity and timeslice
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * nt * Vsh) return;
+    const int par = i / (nt * Vsh);
+    const int cb = par * src_lat.Vh + src_t * Vsh + (i - par * nt * Vsh);  // consecutive threads: consecutive sites
+    const Site st = site_of_cb(src_lat, cb);
+    const int dt = dst_t + (st.c[3] - src_t);
+    const int ds = st.s + (dt - st.c[3]) * dst_lat.stride[3];
+    const int dcb = cb_of(dst_lat, ds, (st.c[0] + st.c[1] + st.c[2] + dt) & 1);
+    for (int k = 0; k < nc; k++) {
+        if (nc == 36 && !((mu_mask >> (k / 9)) & 1u)) continue;
+        dst[unit_index(nc, k, dcb)] = __ldg(src + unit_index(nc, k, cb));
+    }
+}
+
+int launch_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
+                           int dst_t, int nt, int prec, int nc, unsigned mu_mask, cudaStream_t st) {
+    const int n = nt * (src_lat->p.V / src_lat->p.L[3]);
+    const int blocks = (n + 255) / 256;
+    if (prec == QCD_F64)
+        copy_timeslices_kernel<double><<<blocks, 256, 0, st>>>(src_lat->p, (const double2 *)src, src_t, dst_lat->p,
+                                                               (double2 *)dst, dst_t, nt, nc, mu_mask);
+    else
+        copy_timeslices_kernel<float><<<blocks, 256, 0, st>>>(src_lat->p, (const float2 *)src, src_t, dst_lat->p,
+                                                              (float2 *)dst, dst_t, nt, nc, mu_mask);
+    return check_launch("copy_timeslices");
+}
+
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *src, void *dst, bool unpack,
                 cudaStream_t st) {
     const bool matrix = pairs;  // complex-pair layout (colour matrices, spin-colour vectors) or real layout
     const size_t rb = prec == QCD_F64 ? 8 : 4;
     const size_t shm = (size_t)PK_SITES * (ncomp + 2) * rb;
-    if (shm <= 48 * 1024) {  // transpose through shared memory; larger ncomp falls back to the direct kernel
-        const int blocks = (lat->p.V + PK_SITES - 1) / PK_SITES;
-        if (prec == QCD_F64) {
-            if (unpack) pack_tr_kernel<double, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);
-            else pack_tr_kernel<double, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);
-        } else {
-            if (unpack) pack_tr_kernel<float, true><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst);
-            else pack_tr_kernel<float, false><<<blocks, 256, shm, st>>>(lat->p, ncomp, matrix, (const float *)src, (float *)dst);
-        }
-        return check_launch(unpack ? "unpack" : "pack");
-    }
+    if (shm <= 48 * 1024)  // transpose through shared memory; larger ncomp falls back to the direct kernel
+        return launch_pack_range(lat, prec, ncomp, matrix, src, dst, unpack, 0, lat->p.V, st);
     const dim3 grid((lat->p.V + 255) / 256, ncomp < 72 ? ncomp : 72);
     if (prec == QCD_F64) {
         if (unpack) pack_kernel<double, true><<<grid, 256, 0, st>>>(lat->p, ncomp, matrix, (const double *)src, (double *)dst);

@@ -17,6 +17,11 @@ struct LatP {
     int stride[4];  // lexicographic strides 1, Lx, Lx*Ly, Lx*Ly*Lz
     int V;          // sites
     int Vh;         // V/2 sites per parity
+    // domain decomposition in t: a slab lattice stores its timeslices plus a one-site halo on
+    // both sides; the stencil kernels update the interior timeslices [t0, t1) only (a full lattice: 0, Lt), and the
+    // generator is keyed on the GLOBAL lexicographic site (s + site_off) mod gV (a full lattice: 0, V)
+    int t0, t1;
+    int site_off, gV;
 };
 
 // 4-D tile handled by one thread block of the stencil kernels (force).  The block owns the sites
@@ -45,6 +50,7 @@ struct qcd_lattice {
     size_t workspace_doubles;
     int tile_all[4];  // default 4-D block tile of the stencil kernel, subset ALL (both parities per block)
     int tile_par[4];  // the same for one parity (EVEN / ODD)
+    int par_flip;     // slab lattices: 1 if local parity = global parity ^ 1 (subsets are translated at the ABI)
 };
 
 namespace qcd {
@@ -77,6 +83,14 @@ int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p
                      void *Uout, cudaStream_t st);
 // default block tile of the stencil kernels (force.cu), computed once per lattice
 void default_force_tile(const LatP &lat, int npar, int out[4]);
+// copy `nt` timeslices starting at src_t of a pair-layout field with nc units per site into dst (same spatial
+// extents) starting at dst_t; mu_mask (matrix fields, nc = 36): bit mu set = copy link mu
+int launch_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
+                           int dst_t, int nt, int prec, int nc, unsigned mu_mask, cudaStream_t st);
+// timeslices [t_begin, t_begin + nt) only: the canonical side (src when packing, dst when unpacking) holds exactly
+// those sites, the device side is the whole field
+int launch_pack_slab(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *src, void *dst, bool unpack,
+                     int t_begin, int nt, cudaStream_t st);
 int launch_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *F, void *P,
                       cudaStream_t st);
 int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,

@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(128) gauss_field_kernel(const LatP lat, const 
     const int mu = blockIdx.y;
     const Site st = site_of_cb(lat, cb);
     double q[8];
-    gauss8(seed, (uint32_t)st.s, mu, stream_id, KIND == 0 ? 1u : 0u, q);
+    gauss8(seed, global_site(lat, st.s), mu, stream_id, KIND == 0 ? 1u : 0u, q);
     if (KIND == 0) {
         M3<T> P;
         herm_from_coeffs(P, q);
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(128) perturb_kernel(const LatP lat, const uint
     for (int e = 0; e < 9; e++) {
         uint32_t w[4];
         double u[2], g[2];
-        rng_block(seed, (uint32_t)st.s, (uint32_t)(mu * 16 + e), 0u, 2u, w, u, g);
+        rng_block(seed, global_site(lat, st.s), (uint32_t)(mu * 16 + e), 0u, 2u, w, u, g);
         pair_t<T> v = p[e * CHUNK];
         v.x = (T)((double)v.x + sigma * g[0]);
         v.y = (T)((double)v.y + sigma * g[1]);
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(128) spinor_gauss_kernel(const LatP lat, const
     const Site st = site_of_cb(lat, cb);
     uint32_t w[4];
     double u[2], g[2];
-    rng_block(seed, (uint32_t)st.s, (uint32_t)(64 + k), stream_id, 4u, w, u, g);
+    rng_block(seed, global_site(lat, st.s), (uint32_t)(64 + k), stream_id, 4u, w, u, g);
     const double isq2 = 0.70710678118654752440;
     pair_t<T> v;
     v.x = (T)(g[0] * isq2);

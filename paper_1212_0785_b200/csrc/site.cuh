@@ -43,6 +43,11 @@ __device__ __forceinline__ Site site_of_lex(const LatP &lat, int s) {
     return st;
 }
 
+// the generator's site counter: the GLOBAL lexicographic index (slab lattices carry an offset)
+__device__ __forceinline__ uint32_t global_site(const LatP &lat, int s) {
+    return (uint32_t)(((unsigned long long)s + (unsigned long long)lat.site_off) % (unsigned long long)lat.gV);
+}
+
 // lexicographic index change for one periodic hop in +mu / -mu
 __device__ __forceinline__ int dfwd(const LatP &lat, const Site &st, int mu) {
     return st.c[mu] == lat.L[mu] - 1 ? -(lat.L[mu] - 1) * lat.stride[mu] : lat.stride[mu];
