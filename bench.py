@@ -322,7 +322,7 @@ def run_ours(args, cfg):
                      "fma_per_site": FMA_FORCE + FMA_MOM + (FMA_LINK if single else 0),
                      "fma_peak": fma_peak, "fma_peak_source": fma_src},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * fb, "d2h_bytes_per_step": 2 * fb,
-                "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout)"},
+                "steps": Ke, "call": "qcd_md_host (pinned host buffers, canonical layout; H2D, pack, single-pass step, unpack, D2H pipelined over 16 slabs of timeslices on three streams)"},
         "gpu_launches": K if single else 2 * K,
         "clocks": clocks_timed,
     }

@@ -355,9 +355,14 @@ double qcd_probe_work(int what, int prec, int reps);
 int qcd_probe_launch(int what, int prec, int reps, void *scratch, size_t scratch_bytes, void *stream);
 
 /* End-to-end call on HOST buffers (used for the e2e measurement): U_host and P_host are host arrays
- * in the canonical layout (pinned memory makes the copies asynchronous).  Enqueues on `stream`:
- * host->device copies, pack, `nsteps` fused MD steps (eps_p = eps_u = eps), unpack, device->host
- * copies back into U_host and P_host.  device_work: qcd_md_host_work_bytes(lat, prec) device bytes. */
+ * in the canonical layout (pinned memory makes the copies asynchronous).  `nsteps` MD steps (eps_p = eps_u = eps)
+ * between a host->device and a device->host transfer of both fields, results back in U_host and P_host.  As in
+ * PAPER.md:75-79 (section 5.1, transfers overlapped with kernels on CUDA streams) the work runs as a pipeline over
+ * slabs of timeslices on three internal streams — H2D copies; pack, single-pass step per slab, unpack; D2H copies —
+ * so that for one step both PCIe directions are busy at once.  `stream` is joined at entry and at exit with events
+ * (the work is ordered after what `stream` held and before what is enqueued on it next); the host is never
+ * synchronised.  Lattices with fewer than 8 slabs run on `stream` alone.
+ * device_work: qcd_md_host_work_bytes(lat, prec) device bytes. */
 int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host,
                 void *P_host, void *device_work, void *stream);
 

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqcdmd.so")
 BUILD = os.path.join(ROOT, "build", "qcdmd")
-SOURCES = ["api.cu", "force.cu", "update.cu", "random.cu", "reduce.cu", "layout.cu", "tune.cu", "probe.cu"]
+SOURCES = ["api.cu", "force.cu", "update.cu", "random.cu", "reduce.cu", "layout.cu", "tune.cu", "probe.cu", "host_pipeline.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xptxas", "-v", "-Xptxas", "-warn-spills"]

@@ -687,6 +687,9 @@ int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int n
     cudaStream_t st = (cudaStream_t)stream;
     const size_t fb = qcd_field_bytes(lat, prec, 72);                // device field (whole chunks of 32 sites)
     const size_t hb = (size_t)lat->p.V * 72 * real_bytes(prec);      // canonical host array
+    if (md_host_can_pipeline(lat))  // slabs of timeslices on three streams (host_pipeline.cu)
+        return md_host_pipelined(lat, prec, beta, eps, nsteps, U_host, P_host, device_work, fb, st);
+    // small lattices (fewer than 8 slabs): one stream, whole fields
     char *w = (char *)device_work;
     void *stageU = w, *stageP = w + fb, *U = w + 2 * fb, *P = w + 3 * fb;
     cudaError_t e = cudaMemcpyAsync(stageU, U_host, hb, cudaMemcpyHostToDevice, st);

@@ -559,7 +559,8 @@ static ForceSel force_sel(const qcd_lattice *lat, int prec, int subset) {
     TuneCfg cfg;
     if (tune_lookup(lat, prec, subset, QCD_KERNEL_FORCE, cfg)) {
         fs.variant = cfg.variant;
-        if (cfg.tile[0]) t = cfg.tile;  // validated by qcd_tune_set
+        // validated by qcd_tune_set for the lattice it was set on; a view of fewer timeslices keeps its own default
+        if (cfg.tile[0] && (lat->p.t1 - lat->p.t0) % cfg.tile[3] == 0) t = cfg.tile;
     }
     tile_from_extents(lat->p, subset, t, fs.tp);
     return fs;

@@ -121,6 +121,10 @@ int launch_inner_product(const qcd_lattice *lat, int prec, int subset, int nc, c
                          bool per_t, double *out, double *ws, cudaStream_t st);
 int launch_pack(const qcd_lattice *lat, int prec, int ncomp, bool pairs, const void *lex, void *soa, bool unpack,
                 cudaStream_t st);
+// qcd_md_host as a three-stream pipeline over slabs of timeslices (host_pipeline.cu)
+bool md_host_can_pipeline(const qcd_lattice *lat);
+int md_host_pipelined(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host, void *P_host,
+                      void *work, size_t fb, cudaStream_t user);
 // probes of the FMA / L1 / shared-memory / L2 rates (probe.cu)
 double probe_work(int what, int prec, int reps);
 size_t probe_scratch_bytes(int what);

@@ -856,3 +856,45 @@ def test_config_trajectory_full_size_against_oracle(qcd, orc_omp, cfg, prec, n):
         return (g[..., 0] + 1j * g[..., 1]).T.reshape(len(sites), 4, 3, 3)
 
     assert rel(gather(dU), rU[sites]) < TOL[prec] and rel(gather(dP), rP[sites]) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,nsteps", [((8, 8, 8, 16), 1), ((8, 8, 8, 16), 3), ((8, 8, 8, 32), 2), ((6, 4, 2, 8), 1),
+                                         ((8, 8, 8, 16), 0), ((4, 4, 4, 4), 2)])
+def test_md_host_pipeline_matches_the_oracle(qcd, orc_omp, prec, dims, nsteps):
+    """qcd_md_host (the end-to-end call of bench.py) on pinned host buffers: slabs of 1 and 2 timeslices on three
+    streams, one / several / zero steps, and the single-stream path of small lattices, against nsteps oracle MD steps;
+    back-to-back calls on one stream stay ordered"""
+    import torch
+    beta, eps = 5.9, 0.04
+    lat = qcd.Lattice(dims)
+    dt = tdtype(prec)
+    U = round_to(prec, orc_omp.hot_start(dims, 21, 0.5))
+    P = round_to(prec, orc_omp.mom_refresh(dims, 22))
+
+    def to_host(a):
+        return torch.from_numpy(np.ascontiguousarray(a).view(np.float64).reshape(-1)).to(dt).pin_memory()
+
+    hU, hP = to_host(U), to_host(P)
+    p = qcd.F64 if prec == "f64" else qcd.F32
+    work = torch.empty(lat.md_host_work_bytes(p) // hU.element_size(), dtype=dt, device="cuda")
+    qcd.qcd_md_host(lat, hU, hP, beta, eps, nsteps, work)
+    torch.cuda.synchronize()
+    rU, rP = U, P
+    for _ in range(nsteps):
+        rU, rP = orc_omp.md_step(dims, beta, eps, eps, rU, rP)
+
+    def from_host(h):
+        return h.to(torch.float64).numpy().view(np.complex128).reshape(-1, 4, 3, 3)
+
+    if nsteps == 0:
+        assert np.array_equal(from_host(hU), U) and np.array_equal(from_host(hP), P)
+    else:
+        assert rel(from_host(hU), rU) < TOL[prec] and rel(from_host(hP), rP) < TOL[prec]
+    # a second call continues from the first one's output without a host synchronisation in between
+    hU2, hP2 = to_host(U), to_host(P)
+    qcd.qcd_md_host(lat, hU2, hP2, beta, eps, 1, work)
+    qcd.qcd_md_host(lat, hU2, hP2, beta, eps, 1, work)
+    torch.cuda.synchronize()
+    rU, rP = orc_omp.md_step(dims, beta, eps, eps, *orc_omp.md_step(dims, beta, eps, eps, U, P))
+    assert rel(from_host(hU2), rU) < TOL[prec] and rel(from_host(hP2), rP) < TOL[prec]
