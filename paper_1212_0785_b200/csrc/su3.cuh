@@ -36,12 +36,26 @@ __host__ __device__ __forceinline__ unsigned unit_index(int NC, int k, int cb) {
     return ((unsigned)(cb >> 5) * (unsigned)NC + (unsigned)k) * 32u + (unsigned)(cb & 31);
 }
 
+// read-only load that asks L1 to keep the line (ld.global.nc.L1::evict_last, SASS LDG.E.EL.CONSTANT): for the
+// links of the stencil kernels, which neighbouring threads of the block read again within the same direction, while
+// the streaming accesses around them (momenta, outputs: ld/st.global.cs) are marked evict-first
+__device__ __forceinline__ double2 ldg_keep(const double2 *p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::evict_last.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ldg_keep(const float2 *p) {
+    float2 v;
+    asm volatile("ld.global.nc.L1::evict_last.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 template <typename T>
 __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
     const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
 #pragma unroll
     for (int e = 0; e < 9; e++) {
-        pair_t<T> v = __ldg(p + e * CHUNK);
+        pair_t<T> v = ldg_keep(p + e * CHUNK);
         m.re[e] = v.x;
         m.im[e] = v.y;
     }

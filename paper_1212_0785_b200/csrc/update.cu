@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(256) link_update_kernel(const int V, const int
         load_link_rw(R, U, V, mu, cb);
     } else {
         M3<T> Q, Ul, E;
-        load_link(Q, P, V, mu, cb);
+        load_link_cs(Q, P, V, mu, cb);  // touched once: streaming
         load_link_rw(Ul, U, V, mu, cb);
         if (MODE == 1) {
             expi_herm_scaled<2>(E, Q, eps);
