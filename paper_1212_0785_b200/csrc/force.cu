@@ -411,13 +411,18 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
         if (threadIdx.x < 32) tmem_dealloc<TMEM_COLS>(tmem_base);
     }
     if (SUMS) {
+        // one plaquette partial per (timeslice of the tile, block), stored timeslice-major: the partials of one
+        // timeslice are consecutive whatever the tile's t extent (R13); then one K partial per block
         __shared__ double red[FORCE_NT];
-        const double a = block_sum_any<FORCE_NT>(sumW, red);
-        const double b = block_sum_any<FORCE_NT>(sumK, red);
-        if (threadIdx.x == 0) {
-            partial[blockIdx.x] = a;
-            partial[gridDim.x + blockIdx.x] = b;
+        const int nxyz = tile.nt[0] * tile.nt[1] * tile.nt[2];
+        const int bt = blockIdx.x / nxyz, bxyz = blockIdx.x - bt * nxyz;
+        const int jt = st.c[3] - lat.t0 - bt * tile.T[3];
+        for (int q = 0; q < tile.T[3]; q++) {
+            const double a = block_sum_any<FORCE_NT>(jt == q ? sumW : 0.0, red);
+            if (threadIdx.x == 0) partial[(bt * tile.T[3] + q) * nxyz + bxyz] = a;
         }
+        const double b = block_sum_any<FORCE_NT>(sumK, red);
+        if (threadIdx.x == 0) partial[gridDim.x * tile.T[3] + blockIdx.x] = b;
     }
 }
 
@@ -626,12 +631,17 @@ int launch_gauge_force_aniso(const qcd_lattice *lat, int prec, int subset, doubl
                            : launch_force_aniso_t<float>(lat, subset, fs, ws, wt, eps, U, out, fused_mom, st);
 }
 
-// the by-product sums need two doubles of workspace per block of the current launch configuration
+// doubles of workspace the by-product sums write: the plane kernel one plaquette partial per (block, timeslice of
+// its tile) and one K partial per block, the staple kernel two per block
+static size_t force_sums_doubles(const ForceSel &fs) {
+    const size_t blocks = (size_t)fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
+    return blocks * (fs.variant == QCD_FORCE_STAPLE ? 2 : fs.tp.T[3] + 1);
+}
+
 int force_sums_check(const qcd_lattice *lat, int prec) {
     const ForceSel fs = force_sel(lat, prec, QCD_ALL);
-    const size_t blocks = (size_t)fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
-    if (2 * blocks + 8 > lat->workspace_doubles) {
-        set_error("force sums: the workspace cannot hold two doubles per block of the tuned tile");
+    if (force_sums_doubles(fs) + 8 > lat->workspace_doubles) {
+        set_error("force sums: the workspace cannot hold the per-block partials of the tuned tile");
         return QCD_EWORKSPACE;
     }
     return QCD_OK;
@@ -646,13 +656,14 @@ static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, doubl
                                const void *U, void *P, void *Uout, double *out_plaq, double *out_K, double *out_per_t,
                                double *ws, cudaStream_t st) {
     const int blocks = fs.tp.nt[0] * fs.tp.nt[1] * fs.tp.nt[2] * fs.tp.nt[3];
-    if ((size_t)2 * blocks > lat->workspace_doubles) {
+    if (force_sums_doubles(fs) + 8 > lat->workspace_doubles) {
         set_error("force sums: workspace too small");
         return QCD_EWORKSPACE;
     }
     const bool plane = fs.variant != QCD_FORCE_STAPLE;
     const bool slab = lat->p.t0 != 0 || lat->p.t1 != lat->p.L[3];
-    if (out_per_t && !(plane && fs.tp.T[3] == 1 && !slab)) return -1;
+    if (out_per_t && !(plane && !slab)) return -1;
+    const int nW = plane ? blocks * fs.tp.T[3] : blocks;  // plaquette partials
     const T c = (T)(beta / 12.0);
     if (Uout)
         launch_force_k<T, true, true, false, true>(lat, fs, c, (T)eps_p, (const pair_t<T> *)U, (pair_t<T> *)P, (T)eps_u,
@@ -664,12 +675,12 @@ static int launch_force_sums_t(const qcd_lattice *lat, const ForceSel &fs, doubl
     // plane kernel: sum of the six plaquette traces per site; staple kernel: sum_mu Re tr W_mu = 4 x that
     // a slab lattice sums (and averages) over its interior timeslices only
     const double V = (double)(lat->p.V / lat->p.L[3]) * (double)(lat->p.t1 - lat->p.t0);
-    QCD_TRY_RC(launch_sum_partials(ws, 1, blocks, 1.0 / ((plane ? 18.0 : 72.0) * V), out_plaq, st));
-    if (out_per_t) {  // blocks of one timeslice are consecutive (the t index of the tile is the slowest)
+    QCD_TRY_RC(launch_sum_partials(ws, 1, nW, 1.0 / ((plane ? 18.0 : 72.0) * V), out_plaq, st));
+    if (out_per_t) {  // the partials of one timeslice are consecutive (timeslice-major order in the kernel)
         const int Lt = lat->p.L[3];
-        QCD_TRY_RC(launch_sum_partials(ws, Lt, blocks / Lt, (double)Lt / (18.0 * V), out_per_t, st));
+        QCD_TRY_RC(launch_sum_partials(ws, Lt, nW / Lt, (double)Lt / (18.0 * V), out_per_t, st));
     }
-    return launch_sum_partials(ws + blocks, 1, blocks, 1.0, out_K, st);
+    return launch_sum_partials(ws + nW, 1, blocks, 1.0, out_K, st);
 }
 
 int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,

@@ -766,13 +766,15 @@ def oracle_trajectory_observed(orc, dims, beta, eps, n, U, P):
                                                ((8, 8, 8, 16), "f64", 5, None), ((6, 4, 2, 8), "f64", 3, None),
                                                ((8, 8, 8, 16), "f64", 3, (8, 2, 2, 2)), ((8, 8, 8, 16), "f32", 3, None),
                                                ((8, 8, 8, 16), "f64", 4, (8, 4, 4, 1)), ((8, 8, 8, 16), "f32", 2, (8, 4, 4, 1)),
-                                               ((8, 8, 8, 16), "f64", 3, (8, 4, 2, 1)), ((8, 8, 8, 16), "f64", 2, "staple")])
+                                               ((8, 8, 8, 16), "f64", 3, (8, 4, 2, 1)), ((8, 8, 8, 16), "f64", 2, "staple"),
+                                               ((8, 8, 8, 16), "f64", 3, (4, 2, 2, 4)), ((8, 8, 8, 16), "f32", 2, (8, 2, 2, 2)),
+                                               ((4, 6, 2, 8), "f64", 2, (4, 3, 2, 2))])
 def test_trajectory_observables_every_step(qcd, orc_omp, dims, prec, n, tile):
     """qcd_trajectory: final fields and the per-step (plaquette, per-timeslice plaquette, K) series against the
     oracle's leapfrog step by step; odd and even step counts (the ping-pong starts differently), a block that
-    is not a whole number of warps, tiles inside one timeslice (per-timeslice values are by-products of the force
-    kernel), tiles that span two timeslices and the staple variant (they then come from the stand-alone
-    plaquette kernel)"""
+    is not a whole number of warps, tiles inside one timeslice and tiles that span two or four timeslices
+    (per-timeslice values are by-products of the force kernel: one partial per block and timeslice of its tile) and
+    the staple variant (they then come from the stand-alone plaquette kernel)"""
     import torch
     beta, eps = 5.8, 0.05
     lat = qcd.Lattice(dims)
