@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_pass1(const LatP lat, cons
 
 // plaquette pass 1, same chunk geometry and partial layout as reduce_pass1 (grid (cps, nseg, ncomp_out)) but in
 // PLAQ_THREADS-thread blocks, several resident per SM: the stencil kernel wants warps, not wide blocks
-// (profiles/r01c_per_kernel.md).  which0: 0 = all planes; 1 = comp 0 space-space, comp 1 space-time.
+// (profiles/r02_per_kernel.md).  which0: 0 = all planes; 1 = comp 0 space-space, comp 1 space-time.
 constexpr int PLAQ_THREADS = 128;
 template <typename T>
 __global__ void __launch_bounds__(PLAQ_THREADS, 3) plaquette_pass1(const LatP lat, const int which0,
