@@ -3,7 +3,7 @@
 // that bench.py times with CUDA events like any other call (the library never synchronises):
 //   FMA   chains of 3x3 complex products held in registers, no memory: the plain-ALU FMA rate the staple
 //         arithmetic can reach (the same mul<> the force kernel uses)
-//   L1    every block re-reads its own 32 kB with 128-bit loads: L1-resident load bandwidth
+//   L1    every block re-reads its own 64 kB with 128-bit loads: L1-resident load bandwidth
 //   LDS   the same from shared memory
 //   L2    all blocks stream one 48 MB buffer: L2-resident bandwidth as the SMs see it
 #include "qcd_internal.h"
@@ -13,7 +13,7 @@ namespace qcd {
 
 constexpr int PROBE_THREADS = 512;
 constexpr int PROBE_BLOCKS_PER_SM = 2;
-constexpr size_t PROBE_L1_BYTES = 32 * 1024;         // per block
+constexpr size_t PROBE_L1_BYTES = 64 * 1024;         // per block (two blocks per SM: 128 kB, L1-resident)
 constexpr size_t PROBE_LDS_BYTES = 64 * 1024;        // per block
 constexpr size_t PROBE_L2_BYTES = 48ull << 20;       // whole buffer
 
@@ -37,14 +37,22 @@ __global__ void __launch_bounds__(256) probe_fma_kernel(const int reps, const T 
     if (s == T(1.2345)) out[0] = s;  // never true: keeps the chain alive
 }
 
+// eight independent 128-bit loads in flight per thread and iteration (a single dependent load per iteration
+// measures latency, not the data path: 84 instead of 117 B/clk/SM)
 __global__ void probe_l1_kernel(const double2 *__restrict__ p, const size_t n_per_block, const int reps, double2 *out) {
     const double2 *q = p + (size_t)blockIdx.x * n_per_block;
     double2 acc = {0, 0};
+    const size_t bd = blockDim.x;
     for (int r = 0; r < reps; r++)
-        for (size_t i = threadIdx.x; i < n_per_block; i += blockDim.x) {
-            const double2 v = __ldg(q + i);
-            acc.x += v.x;
-            acc.y += v.y;
+        for (size_t i = threadIdx.x; i + 7 * bd < n_per_block; i += 8 * bd) {
+            double2 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) v[u] = __ldg(q + i + u * bd);
+#pragma unroll
+            for (int u = 0; u < 8; u++) {
+                acc.x += v[u].x;
+                acc.y += v[u].y;
+            }
         }
     if (acc.x == 1.2345) out[0] = acc;
 }
@@ -52,13 +60,21 @@ __global__ void probe_l1_kernel(const double2 *__restrict__ p, const size_t n_pe
 __global__ void probe_l2_kernel(const double2 *__restrict__ p, const size_t n, const int reps, double2 *out) {
     double2 acc = {0, 0};
     const size_t start = ((size_t)blockIdx.x * 7919 * 1024) % n;
+    const size_t bd = blockDim.x;
     for (int r = 0; r < reps; r++)
-        for (size_t i = threadIdx.x; i < n / 8; i += blockDim.x) {
-            size_t j = start + i;
-            if (j >= n) j -= n;
-            const double2 v = __ldg(p + j);
-            acc.x += v.x;
-            acc.y += v.y;
+        for (size_t i = threadIdx.x; i + 3 * bd < n / 8; i += 4 * bd) {
+            double2 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                size_t j = start + i + u * bd;
+                if (j >= n) j -= n;
+                v[u] = __ldg(p + j);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                acc.x += v[u].x;
+                acc.y += v[u].y;
+            }
         }
     if (acc.x == 1.2345) out[0] = acc;
 }
