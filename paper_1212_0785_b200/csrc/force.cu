@@ -63,45 +63,13 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
     return st;
 }
 
-// Lexicographic offsets of the periodic hops x -> x +- e_d for the direction d = (mu + k) & 3, k a compile-time
-// constant and mu the (rolled) loop variable.  Picking df[d] from a per-thread register array with a run-time d
-// compiles to branches, which keep the compiler from moving the next product's loads above the current one.  Two
-// ways around it, chosen by precision (measured at 32^3x64, git history of this file: 1.47 -> 1.43 ms in fp64, 0.82 -> 0.80 in fp32):
-//   ROT = true  (fp32: registers to spare, instruction issue is the limit)  the arrays are rotated at the end of
-//               every iteration so that entry k belongs to direction (mu + k) & 3: compile-time indices.
-//   ROT = false (fp64: every register counts)  the two possible hops per direction are block-uniform and sit in
-//               shared memory, tab[d] = stride_d, tab[4 + d] = -(L_d - 1) stride_d; a thread keeps eight wrap bits.
-template <bool ROT>
-struct Hops;
-
-template <>
-struct Hops<true> {
-    int df[4], db[4];
-    __device__ __forceinline__ void init(const LatP &lat, const Site &st, int *) {
-#pragma unroll
-        for (int d = 0; d < 4; d++) {
-            df[d] = dfwd(lat, st, d);
-            db[d] = dbwd(lat, st, d);
-        }
-    }
-    template <int K>
-    __device__ __forceinline__ int fwd(int) const { return df[K]; }
-    template <int K>
-    __device__ __forceinline__ int bwd(int) const { return db[K]; }
-    __device__ __forceinline__ void next() {
-        const int tf = df[0], tb = db[0];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            df[d] = df[d + 1];
-            db[d] = db[d + 1];
-        }
-        df[3] = tf;
-        db[3] = tb;
-    }
-};
-
-template <>
-struct Hops<false> {
+// Lexicographic offsets of the periodic hops x -> x +- e_d for the direction d = (mu + k) & 3, mu the (rolled) loop
+// variable.  Picking them from a per-thread register array with a run-time index compiles to branches, which keep the
+// compiler from moving the next product's loads above the current one.  The two possible hops per direction are
+// block-uniform, so they sit in shared memory, tab[d] = stride_d, tab[4 + d] = -(L_d - 1) stride_d, and a thread keeps
+// eight wrap bits.  (Register arrays rotated once per direction were 2 % faster in fp32 while the plane loop was
+// unrolled; with it rolled the table wins in both precisions: profiles/r02_force_limiters.md.)
+struct Hops {
     const int *tab;  // shared, 8 ints
     unsigned wrap;   // bit d: c[d] == L[d] - 1;  bit 4 + d: c[d] == 0
     // every thread of the block calls init before the first use; the caller synchronises the block
@@ -115,17 +83,14 @@ struct Hops<false> {
 #pragma unroll
         for (int d = 0; d < 4; d++) wrap |= (st.c[d] == lat.L[d] - 1 ? 1u << d : 0u) | (st.c[d] == 0 ? 16u << d : 0u);
     }
-    template <int K>
-    __device__ __forceinline__ int fwd(int mu) const {
-        const int d = (mu + K) & 3;
+    __device__ __forceinline__ int fwd(int mu, int k) const {
+        const int d = (mu + k) & 3;
         return tab[d + 4 * ((wrap >> d) & 1u)];
     }
-    template <int K>
-    __device__ __forceinline__ int bwd(int mu) const {
-        const int d = (mu + K) & 3;
+    __device__ __forceinline__ int bwd(int mu, int k) const {
+        const int d = (mu + k) & 3;
         return -tab[d + 4 * ((wrap >> (4 + d)) & 1u)];
     }
-    __device__ __forceinline__ void next() {}
 };
 
 // Fixed-order sum of one double per thread over a block of ANY size (partial last warp included: no shuffle
@@ -324,7 +289,7 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     __shared__ int hop_tab[8];
     Pend<T, TMEM> pend;
     const Site st = tile_site(lat, tile, threadIdx.x);
-    Hops<sizeof(T) == 4> hop;
+    Hops hop;
     hop.init(lat, st, hop_tab);
     if (TMEM) {
         if (threadIdx.x < 32) tmem_alloc<TMEM_COLS>(&tmem_base);
@@ -344,18 +309,21 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
 
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
-        const int dfm = hop.template fwd<0>(mu);
+        const int dfm = hop.fwd(mu, 0);
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
         M3<T> Pm;
         if (FUSED && EARLYP) load_link_cs(Pm, out, V, mu, cb);
         // planes (mu, nu), nu = mu + k > mu: closed plaquette -> TA parts of W_mu (+) and of W_nu (-)
-#pragma unroll
-        for (int k = 1; k < 4; k++) {
-            if (k > 3 - mu) continue;  // uniform over the grid
+        // this loop is rolled: its bodies are separated by the uniform trip count anyway (nothing is scheduled across
+        // them), and one copy instead of three brings the kernel from 53 to 40 kB of code (instruction cache:
+        // -1.5 % in fp64, -5 % in fp32, profiles/r02_force_limiters.md); the staple loop below stays unrolled
+        // (rolled: +1 % in fp64) because ptxas starts the next staple's loads under the current product
+#pragma unroll 1
+        for (int k = 1; k <= 3 - mu; k++) {
             const int nu = mu + k;
             const T w = ANISO ? (nu == 3 ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;
-            const int cb_pn = cb_of(lat, st.s + (k == 1 ? hop.template fwd<1>(mu) : k == 2 ? hop.template fwd<2>(mu) : hop.template fwd<3>(mu)), par ^ 1);  // x + nu
+            const int cb_pn = cb_of(lat, st.s + hop.fwd(mu, k), par ^ 1);  // x + nu
             M3<T> X, Y, Z;
             load_link(X, U, V, nu, cb_pm);
             load_link(Y, U, V, mu, cb_pn);
@@ -378,7 +346,7 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
             const int nu = (mu + k) & 3;
             const T w = ANISO ? ((mu == 3 || nu == 3) ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;  // warp-uniform
-            const int dbn = k == 1 ? hop.template bwd<1>(mu) : k == 2 ? hop.template bwd<2>(mu) : hop.template bwd<3>(mu);
+            const int dbn = hop.bwd(mu, k);
             const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
             const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
             M3<T> X, Y, Z;
@@ -402,7 +370,6 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
         }
         force_from_ta(F, acc, c);
         finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
-        hop.next();
     }
     if (TMEM) {
         tmem_wait_st();
@@ -435,7 +402,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
     __shared__ int hop_tab[8];
     double sumW = 0.0, sumK = 0.0;
     const Site st = tile_site(lat, tile, threadIdx.x);
-    Hops<sizeof(T) == 4> hop;
+    Hops hop;
     hop.init(lat, st, hop_tab);
     __syncthreads();
     const int V = lat.V;
@@ -444,7 +411,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
 
 #pragma unroll 1
     for (int mu = 0; mu < 4; mu++) {
-        const int dfm = hop.template fwd<0>(mu);
+        const int dfm = hop.fwd(mu, 0);
         const int cb_pm = cb_of(lat, st.s + dfm, par ^ 1);  // x + mu
         M3<T> A, Pm;
         // the momenta come straight from HBM (no reuse): with registers to spare (fp32) their loads are issued
@@ -456,8 +423,8 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
             const int nu = (mu + k) & 3;
             const T w = ANISO ? ((mu == 3 || nu == 3) ? wt : ws) : T(1);
             if (ANISO && w == T(0)) continue;  // warp-uniform
-            const int dfn = k == 1 ? hop.template fwd<1>(mu) : k == 2 ? hop.template fwd<2>(mu) : hop.template fwd<3>(mu);
-            const int dbn = k == 1 ? hop.template bwd<1>(mu) : k == 2 ? hop.template bwd<2>(mu) : hop.template bwd<3>(mu);
+            const int dfn = hop.fwd(mu, k);
+            const int dbn = hop.bwd(mu, k);
             const int cb_pn = cb_of(lat, st.s + dfn, par ^ 1);      // x + nu
             const int cb_mn = cb_of(lat, st.s + dbn, par ^ 1);      // x - nu
             const int cb_pmmn = cb_of(lat, st.s + dfm + dbn, par);  // x + mu - nu
@@ -485,7 +452,6 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
         project_force(F, W, c);
         if (SUMS) sumW += (double)W.re[0] + (double)W.re[4] + (double)W.re[8];
         finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
-        hop.next();
     }
     if (SUMS) {
         __shared__ double red[FORCE_NT];
