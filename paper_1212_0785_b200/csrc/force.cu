@@ -115,6 +115,21 @@ __device__ __forceinline__ double block_sum_any(double v, double *buf) {
     return r;
 }
 
+// The same for blocks of whole warps (at most 32 of them): shuffle tree per warp, then the warp sums in warp order.
+// buf: 32 doubles of shared memory (the NT-double buffer of block_sum_any would move the L1 carve-out of the
+// stencil kernels: profiles/r02_force_limiters.md section 4).
+__device__ __forceinline__ double block_sum_warps(double v, double *buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    __syncthreads();  // buf may still be read from a previous call
+    if ((threadIdx.x & 31) == 0) buf[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) r += buf[w];
+    return r;
+}
+
 // the momentum update, the sums and the link update that follow the force of one direction (shared by both kernels)
 template <typename T, bool FUSED, bool EARLYP, bool LINK, bool SUMS>
 __device__ __forceinline__ void finish_direction(const M3<T> &F, const M3<T> &Pm, const M3<T> &Um, const T eps,
@@ -130,12 +145,11 @@ __device__ __forceinline__ void finish_direction(const M3<T> &F, const M3<T> &Pm
             P.im[e] = fma_(eps, F.im[e], P.im[e]);
         }
         store_link_cs(P, out, V, mu, cb);
-        if (SUMS) {
+        if (SUMS) {  // |P_mu(x)|^2 in the field's precision (R14), accumulated over links and sites in fp64 (R12)
+            T k2 = T(0);
 #pragma unroll
-            for (int e = 0; e < 9; e++) {
-                sumK = fma((double)P.re[e], (double)P.re[e], sumK);
-                sumK = fma((double)P.im[e], (double)P.im[e], sumK);
-            }
+            for (int e = 0; e < 9; e++) k2 = fma_(P.re[e], P.re[e], fma_(P.im[e], P.im[e], k2));
+            sumK += (double)k2;
         }
         if (LINK) {
             M3<T> E, R;
@@ -380,15 +394,16 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     if (SUMS) {
         // one plaquette partial per (timeslice of the tile, block), stored timeslice-major: the partials of one
         // timeslice are consecutive whatever the tile's t extent (R13); then one K partial per block
-        __shared__ double red[FORCE_NT];
+        __shared__ double red[TMEM ? 32 : FORCE_NT];  // TMEM: the block is whole warps
         const int nxyz = tile.nt[0] * tile.nt[1] * tile.nt[2];
         const int bt = blockIdx.x / nxyz, bxyz = blockIdx.x - bt * nxyz;
         const int jt = st.c[3] - lat.t0 - bt * tile.T[3];
         for (int q = 0; q < tile.T[3]; q++) {
-            const double a = block_sum_any<FORCE_NT>(jt == q ? sumW : 0.0, red);
+            const double v = jt == q ? sumW : 0.0;
+            const double a = TMEM ? block_sum_warps(v, red) : block_sum_any<FORCE_NT>(v, red);
             if (threadIdx.x == 0) partial[(bt * tile.T[3] + q) * nxyz + bxyz] = a;
         }
-        const double b = block_sum_any<FORCE_NT>(sumK, red);
+        const double b = TMEM ? block_sum_warps(sumK, red) : block_sum_any<FORCE_NT>(sumK, red);
         if (threadIdx.x == 0) partial[gridDim.x * tile.T[3] + blockIdx.x] = b;
     }
 }
