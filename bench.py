@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — MD-step site-updates/s of the fused hot path (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--dims Lx,Ly,Lz,Lt]
 
 A "step" is one fused molecular-dynamics step on the whole lattice: P += eps F(U), then
 U <- reunit(exp(i eps P) U) — force, projection, momentum update, exponential, link update and
@@ -468,6 +468,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
+    ap.add_argument("--dims", default=None,
+                    help="Lx,Ly,Lz,Lt: another lattice shape with the parameters of --config (shape studies; the "
+                         "headline workload is the default)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--path", default="single_pass", choices=["two_kernel", "single_pass"],
                     help="single_pass (default, the faster one as measured): qcd_md_step_single_pass ping-ponging two "
@@ -483,7 +486,10 @@ def main():
                          "launches (SURVEY.md 8(d), config 3 row); prints one JSON object with the table")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    cfg = CONFIGS[args.config]
+    cfg = dict(CONFIGS[args.config])
+    if args.dims:
+        cfg["dims"] = tuple(int(x) for x in args.dims.split(","))
+        cfg["name"] = "x".join(str(d) for d in cfg["dims"])
     if args.impl == "reference":
         run_reference(args, cfg)
     elif args.peaks:

@@ -32,8 +32,24 @@ namespace qcd {
 
 constexpr int FORCE_NT = 128;  // threads per block of the stencil kernels (168 registers in fp64 -> 3 blocks per SM)
 
-// thread -> site of the block's tile
-__device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, int j) {
+// Launch order -> canonical block index bx + nt0 (by + nt1 (bz + nt2 bt)).  On lattices whose timeslices are large
+// the blocks are launched z-block by z-block: inside a z-block of tile.zb tiles the order is x, y, z, t, so the
+// links a block shares with its t and z neighbours are still in L2 when they are needed again, because T3 + 2
+// timeslices of the z-block, not of the whole lattice, pass through it (host side: tile_from_extents).
+__device__ __forceinline__ int canonical_block(const TileP &tile, int b) {
+    if (tile.zb == tile.nt[2]) return b;
+    const int nxy = tile.nt[0] * tile.nt[1];
+    const int nin = nxy * tile.zb;
+    const int q = b / (nin * tile.nt[3]);
+    int r = b - q * nin * tile.nt[3];
+    const int bt = r / nin;
+    r -= bt * nin;
+    const int bz = q * tile.zb + r / nxy;
+    return (r % nxy) + nxy * (bz + tile.nt[2] * bt);
+}
+
+// thread -> site of the tile of (canonical) block b
+__device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, int j, int b) {
     int par = tile.par0;
     if (tile.npar == 2) {
         par = j >= tile.tsp ? 1 : 0;
@@ -46,7 +62,6 @@ __device__ __forceinline__ Site tile_site(const LatP &lat, const TileP &tile, in
     r /= tile.T[1];
     const int jz = r % tile.T[2];
     const int jt = r / tile.T[2];
-    int b = blockIdx.x;
     const int bx = b % tile.nt[0];
     b /= tile.nt[0];
     const int by = b % tile.nt[1];
@@ -302,7 +317,8 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     __shared__ uint32_t tmem_base;
     __shared__ int hop_tab[8];
     Pend<T, TMEM> pend;
-    const Site st = tile_site(lat, tile, threadIdx.x);
+    const int bc = canonical_block(tile, blockIdx.x);
+    const Site st = tile_site(lat, tile, threadIdx.x, bc);
     Hops hop;
     hop.init(lat, st, hop_tab);
     if (TMEM) {
@@ -396,7 +412,7 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
         // timeslice are consecutive whatever the tile's t extent (R13); then one K partial per block
         __shared__ double red[TMEM ? 32 : FORCE_NT];  // TMEM: the block is whole warps
         const int nxyz = tile.nt[0] * tile.nt[1] * tile.nt[2];
-        const int bt = blockIdx.x / nxyz, bxyz = blockIdx.x - bt * nxyz;
+        const int bt = bc / nxyz, bxyz = bc - bt * nxyz;
         const int jt = st.c[3] - lat.t0 - bt * tile.T[3];
         for (int q = 0; q < tile.T[3]; q++) {
             const double v = jt == q ? sumW : 0.0;
@@ -404,7 +420,7 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
             if (threadIdx.x == 0) partial[(bt * tile.T[3] + q) * nxyz + bxyz] = a;
         }
         const double b = TMEM ? block_sum_warps(sumK, red) : block_sum_any<FORCE_NT>(sumK, red);
-        if (threadIdx.x == 0) partial[gridDim.x * tile.T[3] + blockIdx.x] = b;
+        if (threadIdx.x == 0) partial[gridDim.x * tile.T[3] + bc] = b;
     }
 }
 
@@ -416,7 +432,7 @@ __global__ void __launch_bounds__(FORCE_NT, 3)
                  pair_t<T> *__restrict__ Uout, const T ws, const T wt, double *__restrict__ partial) {
     __shared__ int hop_tab[8];
     double sumW = 0.0, sumK = 0.0;
-    const Site st = tile_site(lat, tile, threadIdx.x);
+    const Site st = tile_site(lat, tile, threadIdx.x, blockIdx.x);
     Hops hop;
     hop.init(lat, st, hop_tab);
     __syncthreads();
@@ -489,7 +505,7 @@ static int divisors(int n, bool even, int *out) {
     return k;
 }
 
-static void tile_from_extents(const LatP &lat, int subset, const int t[4], TileP &tp) {
+static void tile_from_extents(const LatP &lat, int prec, int subset, const int t[4], TileP &tp) {
     tp.npar = subset == QCD_ALL ? 2 : 1;
     tp.par0 = subset == QCD_ODD ? 1 : 0;
     for (int d = 0; d < 4; d++) {
@@ -497,6 +513,19 @@ static void tile_from_extents(const LatP &lat, int subset, const int t[4], TileP
         tp.nt[d] = (d == 3 ? lat.t1 - lat.t0 : lat.L[d]) / t[d];
     }
     tp.tsp = (tp.T[0] / 2) * tp.T[1] * tp.T[2] * tp.T[3];
+    // Launch order (canonical_block).  While a row of tiles in t is worked on, T3 + 2 timeslices of the gauge field
+    // are live in L2; measured on B200 the step loses 11 ... 23 % per site once they exceed about 60 MB (32^3 x Lt
+    // is below: plain order).  Above, z-blocks are cut so that the live part — (z extent + 2) planes of T3 + 2
+    // timeslices — stays under 48 MB: -11 % at 32x64x64x32 and 64^3x32, -3 % at 48^3x96 (profiles/r02_shapes.md).
+    tp.zb = tp.nt[2];
+    const double plane = (double)lat.L[0] * lat.L[1] * (tp.T[3] + 2) * 72.0 * (prec == QCD_F64 ? 8 : 4);
+    if (plane * lat.L[2] > 60e6) {
+        for (int z = tp.nt[2]; z >= 1; z--)
+            if (tp.nt[2] % z == 0 && (z == 1 || plane * (z * tp.T[2] + 2) <= 48e6)) {
+                tp.zb = z;
+                break;
+            }
+    }
 }
 
 // Tile extents dividing L with T0 even and threads = T0/2*T1*T2*T3*npar as close to FORCE_NT as possible (never
@@ -548,7 +577,7 @@ static ForceSel force_sel(const qcd_lattice *lat, int prec, int subset) {
         // validated by qcd_tune_set for the lattice it was set on; a view of fewer timeslices keeps its own default
         if (cfg.tile[0] && (lat->p.t1 - lat->p.t0) % cfg.tile[3] == 0) t = cfg.tile;
     }
-    tile_from_extents(lat->p, subset, t, fs.tp);
+    tile_from_extents(lat->p, prec, subset, t, fs.tp);
     return fs;
 }
 

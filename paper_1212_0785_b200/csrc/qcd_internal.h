@@ -32,6 +32,7 @@ struct TileP {
     int tsp;    // sites per parity per tile = T0/2*T1*T2*T3
     int npar;   // parities per block: 2 (subset ALL) or 1
     int par0;   // parity handled when npar == 1
+    int zb;     // launch order of the plane kernel: z-blocks of zb tiles (nt[2]: plain x, y, z, t order)
 };
 
 // Reduction geometry (fixed, independent of any tuning, so results are run-to-run identical).
