@@ -338,6 +338,18 @@ int qcd_lattice_view_t(const qcd_lattice *lat, int t0, int t1, qcd_lattice **out
 int qcd_lattice_dims(const qcd_lattice *lat, int dims[4], int interior_t[2]);
 int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
                         int dst_t, int nt, int prec, int ncomp, unsigned mu_mask, void *stream);
+/* Link update fused with the halo transport (SURVEY.md 8(e) "peer stores"): on the interior timeslices
+ * [t0, t1) of the slab lattice (or view) `lat`, U <- exp(i eps P) U, reunitarised if reunit != 0 [O8, O9], all four
+ * links of every site; the new links of the slab's first interior timeslice (te = 1) are ALSO stored into the upper
+ * halo of the lower neighbour's gauge field lo_U (links mu = 0..2) and those of its last interior timeslice into the
+ * lower halo of hi_U (all four links) by the thread that computed them — one kernel instead of the link update
+ * followed by two qcd_copy_timeslices.  lo_lat / hi_lat: the neighbours' slab lattices (same spatial extents,
+ * QCD_EDIMS otherwise; t extents may differ); lo_U / hi_U device pointers that may be peer-GPU memory; a neighbour may
+ * be NULL (lattice and field together) and may be this slab itself (one slab: its halos mirror its own boundary).
+ * The slab's own halo timeslices are not written: the neighbours' calls write them, so the caller orders the calls
+ * of different slabs before the next force evaluation (stream or event dependencies), nothing else. */
+int qcd_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
+                         const qcd_lattice *lo_lat, void *lo_U, const qcd_lattice *hi_lat, void *hi_U, void *stream);
 
 /* ---- measured denominators ("Measure DFMA/FFMA peaks with a probe") --------------------
  * One kernel launch per probe, enqueued on `stream` like every other call and timed by the caller with CUDA

@@ -658,6 +658,30 @@ int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, 
                                   (cudaStream_t)stream);
 }
 
+int qcd_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
+                         const qcd_lattice *lo_lat, void *lo_U, const qcd_lattice *hi_lat, void *hi_U, void *stream) {
+    const char *fn = "qcd_link_update_push";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_alias(P, U, qcd_field_bytes(lat, prec, 72), fn));
+    if (lat->p.L[3] < 3 || lat->p.t0 < 1 || lat->p.t1 > lat->p.L[3] - 1)
+        return bad(QCD_EINVAL, "%s: needs a slab lattice (halo timeslices on both sides) or a view of one", fn);
+    const qcd_lattice *nb[2] = {lo_lat, hi_lat};
+    void *nbU[2] = {lo_U, hi_U};
+    for (int k = 0; k < 2; k++) {
+        if ((nb[k] == nullptr) != (nbU[k] == nullptr)) return bad(QCD_EINVAL, "%s: a neighbour needs both its lattice and its field", fn);
+        if (!nb[k]) continue;
+        QCD_TRY(check_common(nb[k], prec, fn));
+        QCD_TRY(check_ptr(nbU[k], fn));
+        if (nb[k]->p.L[3] < 3) return bad(QCD_EINVAL, "%s: a neighbour is not a slab lattice", fn);
+        for (int d = 0; d < 3; d++)
+            if (nb[k]->p.L[d] != lat->p.L[d]) return bad(QCD_EDIMS, "%s: a neighbour differs in a spatial extent", fn);
+        if (nbU[k] == P) return bad(QCD_EALIAS, "%s: a neighbour's gauge field is this slab's momentum field", fn);
+    }
+    return launch_link_update_push(lat, prec, eps, P, U, reunit ? 1 : 0, lo_lat, lo_U, hi_lat, hi_U, (cudaStream_t)stream);
+}
+
 size_t qcd_probe_scratch_bytes(int what) {
     return what >= QCD_PROBE_FMA && what <= QCD_PROBE_L2 ? probe_scratch_bytes(what) : 0;
 }

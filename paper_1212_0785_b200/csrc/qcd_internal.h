@@ -96,6 +96,10 @@ int launch_mom_update(const qcd_lattice *lat, int prec, int subset, double eps, 
                       cudaStream_t st);
 int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps, const void *P, void *U,
                        int mode /*0 exp, 1 exp+reunit, 2 reunit only*/, cudaStream_t st);
+// link update of the interior timeslices of a slab fused with the stores of its boundary timeslices into the
+// neighbours' halos (update.cu)
+int launch_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
+                            const qcd_lattice *lo, void *lo_U, const qcd_lattice *hi, void *hi_U, cudaStream_t st);
 int launch_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed, uint32_t stream_id, void *P,
                        cudaStream_t st);
 int launch_hot_start(const qcd_lattice *lat, int prec, uint64_t seed, double sigma, void *U, cudaStream_t st);

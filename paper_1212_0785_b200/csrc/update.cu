@@ -34,6 +34,49 @@ __global__ void __launch_bounds__(256) link_update_kernel(const int V, const int
     store_link(R, U, V, mu, cb);
 }
 
+// Link update of the interior timeslices of a slab lattice fused with the halo transport ("one
+// exchange per force evaluation ... over NVLink peer stores"): the thread that has the new link of a
+// boundary timeslice in registers also stores it into the neighbour's halo — the first interior timeslice (te = 1)
+// into the upper halo of `lo` (spatial links only: nobody reads a halo's time links from below), the last interior
+// timeslice into the lower halo of `hi` (all four).  lo_U / hi_U may be peer-GPU memory or NULL.  The slab's own
+// halos are NOT written (the neighbours' launches write them).  MODE as in link_update_kernel (0 or 1).
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) link_update_push_kernel(const LatP lat, const T eps,
+                                                               const pair_t<T> *__restrict__ P,
+                                                               pair_t<T> *__restrict__ U, const LatP lo,
+                                                               pair_t<T> *__restrict__ lo_U, const LatP hi,
+                                                               pair_t<T> *__restrict__ hi_U) {
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= lat.V) return;
+    const Site st = site_of_cb(lat, cb);
+    const int t = st.c[3];
+    if (t < lat.t0 || t >= lat.t1) return;
+    const int mu = blockIdx.y;
+    M3<T> Q, Ul, E, R;
+    load_link_cs(Q, P, lat.V, mu, cb);
+    load_link_rw(Ul, U, lat.V, mu, cb);
+    if (MODE == 1) {
+        expi_herm_scaled<2>(E, Q, eps);
+        mul_top2(R, E, Ul);
+        reunit(R);
+    } else {
+        expi_herm_scaled<3>(E, Q, eps);
+        mul<false, false, false>(R, E, Ul);
+    }
+    store_link(R, U, lat.V, mu, cb);
+    const int sx = st.c[0] + lat.L[0] * (st.c[1] + lat.L[1] * st.c[2]);  // spatial index, the same on every slab
+    const int Vs = lat.L[0] * lat.L[1] * lat.L[2];
+    if (t == 1 && lo_U != nullptr && mu < 3) {
+        const int tp = lo.L[3] - 1;
+        const int par = (st.c[0] + st.c[1] + st.c[2] + tp) & 1;
+        store_link(R, lo_U, lo.V, mu, par * lo.Vh + ((sx + Vs * tp) >> 1));
+    }
+    if (t == lat.L[3] - 2 && hi_U != nullptr) {
+        const int par = (st.c[0] + st.c[1] + st.c[2]) & 1;  // tp = 0
+        store_link(R, hi_U, hi.V, mu, par * hi.Vh + (sx >> 1));
+    }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) mom_update_kernel(const int V, const int begin, const int count, const T eps,
                                                          const pair_t<T> *__restrict__ F, pair_t<T> *__restrict__ P) {
@@ -79,6 +122,28 @@ int launch_link_update(const qcd_lattice *lat, int prec, int subset, double eps,
                        cudaStream_t st) {
     return prec == QCD_F64 ? launch_link_update_t<double>(lat, subset, eps, P, U, mode, st)
                            : launch_link_update_t<float>(lat, subset, eps, P, U, mode, st);
+}
+
+template <typename T>
+static int launch_link_update_push_t(const qcd_lattice *lat, double eps, const void *P, void *U, int reunit,
+                                     const qcd_lattice *lo, void *lo_U, const qcd_lattice *hi, void *hi_U,
+                                     cudaStream_t st) {
+    const int threads = 128;
+    const dim3 grid((lat->p.V + threads - 1) / threads, 4);
+    const LatP &pl = lo ? lo->p : lat->p, &ph = hi ? hi->p : lat->p;
+    if (reunit)
+        link_update_push_kernel<T, 1><<<grid, threads, 0, st>>>(lat->p, (T)eps, (const pair_t<T> *)P, (pair_t<T> *)U, pl,
+                                                                (pair_t<T> *)lo_U, ph, (pair_t<T> *)hi_U);
+    else
+        link_update_push_kernel<T, 0><<<grid, threads, 0, st>>>(lat->p, (T)eps, (const pair_t<T> *)P, (pair_t<T> *)U, pl,
+                                                                (pair_t<T> *)lo_U, ph, (pair_t<T> *)hi_U);
+    return check_launch("link_update_push");
+}
+
+int launch_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
+                            const qcd_lattice *lo, void *lo_U, const qcd_lattice *hi, void *hi_U, cudaStream_t st) {
+    return prec == QCD_F64 ? launch_link_update_push_t<double>(lat, eps, P, U, reunit, lo, lo_U, hi, hi_U, st)
+                           : launch_link_update_push_t<float>(lat, eps, P, U, reunit, lo, lo_U, hi, hi_U, st);
 }
 
 template <typename T>

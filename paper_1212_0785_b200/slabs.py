@@ -194,12 +194,35 @@ class SlabSet:
             for v in s.edges:
                 qcd.qcd_force_mom_update(v, s.U, s.P, beta, eps)
 
-    def leapfrog(self, beta, eps, nsteps, overlap=False):
-        self.kick(beta, 0.5 * eps, overlap)
+    def push_update(self, eps, overlap):
+        """link update of every slab fused with the halo transport (qcd_link_update_push): the thread that computes a
+        link of a boundary timeslice also stores it into the neighbour's halo.  overlap = True: the boundary
+        timeslices go first, so their stores travel while the inner timeslices are updated"""
+        n = len(self.slabs)
+        views = (lambda s: list(s.edges) + [s.inner]) if overlap and all(s.inner is not None for s in self.slabs) \
+            else (lambda s: [s.lat])
+        for which in range(len(views(self.slabs[0]))):
+            for r, s in enumerate(self.slabs):
+                up, lo = self.slabs[(r + 1) % n], self.slabs[(r - 1) % n]
+                self.qcd.qcd_link_update_push(views(s)[which], s.P, s.U, eps, True, lo.lat, lo.U, up.lat, up.U)
+
+    def force(self, beta, eps):
+        for s in self.slabs:
+            self.qcd.qcd_force_mom_update(s.lat, s.U, s.P, beta, eps)
+
+    def leapfrog(self, beta, eps, nsteps, overlap=False, fused=False):
+        """fused = False: link update, then qcd_copy_timeslices into the neighbours' halos, then the force;
+        fused = True: the link update stores the boundary timeslices into the neighbours' halos itself"""
+        self.kick(beta, 0.5 * eps, overlap)  # halos are valid after start(): the exchange inside is a no-op in effect
         for k in range(nsteps):
-            for s in self.slabs:
-                self.qcd.qcd_link_update(s.lat, s.P, s.U, eps, reunit=True)
-            self.kick(beta, 0.5 * eps if k == nsteps - 1 else eps, overlap)
+            e = 0.5 * eps if k == nsteps - 1 else eps
+            if fused:
+                self.push_update(eps, overlap)
+                self.force(beta, e)
+            else:
+                for s in self.slabs:
+                    self.qcd.qcd_link_update(s.lat, s.P, s.U, eps, reunit=True)
+                self.kick(beta, e, overlap)
 
     def gather(self, which):
         """interior timeslices of every slab as one canonical host array [V,4,3,3] of the global lattice"""

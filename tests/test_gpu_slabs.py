@@ -63,10 +63,14 @@ def test_generator_is_decomposition_independent(qcd, orc_omp, dims, nslabs, prec
         assert np.array_equal(host(qcd, lat, U), slab_rows(host(qcd, full, fU2), dims, tb, tc))
 
 
+@pytest.mark.parametrize("fused", [False, True])
 @pytest.mark.parametrize("dims,nslabs,prec,overlap", [((8, 8, 8, 16), 2, "f64", False), ((8, 8, 8, 16), 4, "f64", True),
                                                       ((16, 16, 16, 32), 4, "f64", True), ((16, 16, 16, 32), 2, "f32", True),
-                                                      ((8, 8, 8, 16), 1, "f64", False), ((4, 6, 2, 8), 2, "f64", True)])
-def test_slab_trajectory_equals_the_whole_lattice(qcd, orc_omp, dims, nslabs, prec, overlap):
+                                                      ((8, 8, 8, 16), 1, "f64", False), ((4, 6, 2, 8), 2, "f64", True),
+                                                      ((8, 8, 8, 16), 3, "f64", True)])
+def test_slab_trajectory_equals_the_whole_lattice(qcd, orc_omp, dims, nslabs, prec, overlap, fused):
+    """fused = True: the halo transport is done by the link update itself (qcd_link_update_push: the thread that has a
+    boundary link in registers stores it into the neighbour's halo) instead of qcd_copy_timeslices"""
     import torch
     from paper_1212_0785_b200 import slabs
     beta, eps, n, seed = 5.8, 0.05, 3, 0x1212078500000002
@@ -79,7 +83,7 @@ def test_slab_trajectory_equals_the_whole_lattice(qcd, orc_omp, dims, nslabs, pr
     qcd.qcd_leapfrog(full, fU, fP, beta, eps, n)
     ss = slabs.SlabSet(qcd, dims, nslabs, dt)
     ss.start(seed, 0.5)
-    ss.leapfrog(beta, eps, n, overlap=overlap)
+    ss.leapfrog(beta, eps, n, overlap=overlap, fused=fused)
     torch.cuda.synchronize()
     gU, gP = ss.gather("U"), ss.gather("P")
     # the same arithmetic per site whatever the decomposition: bit-identical to the undecomposed run
@@ -100,6 +104,35 @@ def test_slab_trajectory_equals_the_whole_lattice(qcd, orc_omp, dims, nslabs, pr
     ss.exchange()
     qcd.qcd_force_mom_update_sums(s.lat, s.U, s.P, beta, 0.0, out, s.ws)
     assert abs(out[0].item() - rper_t[s.t_begin: s.t_begin + s.n].mean()) < TOL[prec]
+
+
+def test_link_update_push_arguments_and_halo_only_stores(qcd):
+    """argument checks before anything is enqueued; the push writes the neighbours' halos and nothing else of them,
+    and leaves the slab's own halos alone"""
+    import torch
+    a, b = qcd.Lattice((8, 8, 8, 16), slab=(0, 8)), qcd.Lattice((8, 8, 8, 16), slab=(8, 8))
+    c, full = qcd.Lattice((8, 8, 4, 16), slab=(0, 8)), qcd.Lattice((8, 8, 8, 16))
+    Ua, Pa, Ub = a.new_matrix_field(), a.new_matrix_field(), b.new_matrix_field()
+    Uc, Uf, Pf = c.new_matrix_field(), full.new_matrix_field(), full.new_matrix_field()
+    for args, code in (((a, Pa, Ua, 0.1, True, c, Uc, b, Ub), qcd.EDIMS), ((a, Pa, Ua, 0.1, True, b, None, b, Ub), qcd.EINVAL),
+                       ((full, Pf, Uf, 0.1, True, None, None, None, None), qcd.EINVAL),
+                       ((a, Pa, Pa, 0.1, True, None, None, None, None), qcd.EALIAS)):
+        with pytest.raises(qcd.QcdError) as e:
+            qcd.qcd_link_update_push(*args)
+        assert e.value.code == code
+    qcd.qcd_hot_start(a, Ua, 5, 0.5)
+    qcd.qcd_mom_refresh(a, Pa, 5)
+    Ub.fill_(7.0)
+    ref = Ua.clone()
+    qcd.qcd_link_update(a, Pa, ref, 0.1, reunit=True)
+    before = qcd.field_to_host(a, Ua).reshape(10, 512, 4, 3, 3)
+    qcd.qcd_link_update_push(a, Pa, Ua, 0.1, True, b, Ub, b, Ub)
+    got, want = qcd.field_to_host(a, Ua).reshape(10, 512, 4, 3, 3), qcd.field_to_host(a, ref).reshape(10, 512, 4, 3, 3)
+    assert np.array_equal(got[1:9], want[1:9]) and np.array_equal(got[0], before[0]) and np.array_equal(got[9], before[9])
+    nb = qcd.field_to_host(b, Ub).reshape(10, 512, 4, 3, 3)
+    assert np.array_equal(nb[0], want[8])                      # my last interior timeslice -> its lower halo, all links
+    assert np.array_equal(nb[9][:, :3], want[1][:, :3])        # my first -> its upper halo, spatial links
+    assert np.all(nb[1:9] == 7.0 + 7.0j) and np.all(nb[9][:, 3] == 7.0 + 7.0j)
 
 
 def test_copy_timeslices_arguments(qcd):
