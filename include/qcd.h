@@ -314,7 +314,7 @@ int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, c
  * extents.  Semantics of every call on a slab lattice:
  *   - the stencil calls (qcd_gauge_force*, qcd_force_mom_update*, qcd_md_step*, qcd_leapfrog*) update the INTERIOR
  *     timeslices only and read the halos, which the caller refreshes with qcd_copy_timeslices after every link
- *     update (one exchange per force evaluation: from the lower neighbour's last interior timeslice into te = 0,
+ *     update (or which qcd_link_update_push, the link update fused with that transport, has already written) (one exchange per force evaluation: from the lower neighbour's last interior timeslice into te = 0,
  *     all four links; from the upper neighbour's first interior timeslice into te = t_count + 1, mu_mask 0x7);
  *   - the site-local calls act on all stored timeslices (halo values are recomputed or overwritten by the next
  *     exchange); EVEN / ODD always mean the GLOBAL parity;
