@@ -511,6 +511,35 @@ def test_md_step_single_pass(qcd, orc_omp, prec, dims):
     assert e.value.code == qcd.EALIAS
 
 
+def test_z_blocked_launch_order_whole_field(qcd, orc_omp):
+    """32x32x48x8 fp64: three timeslices of U are 85 MB, above the threshold at which the plane kernel launches its
+    blocks z-block by z-block (force.cu: canonical_block, two z-blocks of 24 planes here).  Whole-field comparison of
+    the single-pass step and of the by-product sums (global, per timeslice, K) of one trajectory step: every tile is
+    visited exactly once and its partial sums land in their timeslice's slot"""
+    import torch
+    dims, beta, eps = (32, 32, 48, 8), 5.9, 0.04
+    lat = qcd.Lattice(dims)
+    U = orc_omp.hot_start(dims, 91, 0.4)
+    P = orc_omp.mom_refresh(dims, 92)
+    dU, dP, dV = dev(qcd, lat, U, "f64"), dev(qcd, lat, P, "f64"), lat.new_matrix_field(torch.float64)
+    dV.fill_(float("nan"))
+    qcd.qcd_md_step_single_pass(lat, dU, dP, dV, beta, eps, eps)
+    P1 = orc_omp.mom_update(dims, eps, orc_omp.gauge_force(dims, beta, U), P)
+    U1 = orc_omp.link_update(dims, eps, P1, U, reunit=True)
+    assert rel(host(qcd, lat, dP), P1) < TOL["f64"] and rel(host(qcd, lat, dV), U1) < TOL["f64"]
+    # one trajectory step with observables from the same kernel
+    dU2, dP2 = dev(qcd, lat, U, "f64"), dev(qcd, lat, P, "f64")
+    ws = lat.new_workspace()
+    obs = torch.zeros((2, 2), dtype=torch.float64, device="cuda")
+    per_t = torch.zeros((2, dims[3]), dtype=torch.float64, device="cuda")
+    qcd.qcd_trajectory(lat, dU2, dP2, dV, beta, eps, 1, obs, per_t, ws)
+    rplaq, rper_t = orc_omp.plaquette(dims, U)
+    o = obs.cpu().numpy()
+    assert abs(o[0, 0] - rplaq) < TOL["f64"] and np.abs(per_t[0].cpu().numpy() - rper_t).max() < TOL["f64"]
+    rK = orc_omp.sum(dims, O.SUM_NORM2, P.view(np.float64).reshape(lat.V, 72))[0]
+    assert abs(o[0, 1] - rK) < TOL["f64"] * rK
+
+
 @pytest.mark.parametrize("prec,nsteps", [("f64", 1), ("f64", 4), ("f64", 5), ("f32", 3)])
 def test_leapfrog_single_pass_matches_oracle_trajectory(qcd, orc_omp, prec, nsteps):
     c = inputs.CONFIGS[2]
