@@ -387,6 +387,40 @@ def run_peaks(args):
     print(json.dumps({"peaks": out, "how": "qcd_probe_launch through the C ABI, CUDA events, best of 3 per probe"}), flush=True)
 
 
+def run_slabs(args, cfg):
+    """the single-pass step on the lattice cut into --slabs slabs of timeslices in ONE process on one GPU, halos written
+    by the step kernel of the neighbouring slab (qcd_md_step_single_pass_push): what the
+    decomposition itself costs (halo timeslices, smaller launches, the push stores) with the transport at device-memory
+    speed.  One JSON object; not the headline line."""
+    import torch
+
+    from paper_1212_0785_b200 import binding as qcd
+    from paper_1212_0785_b200 import slabs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dtype = torch.float64 if args.dtype == "f64" else torch.float32
+    dims, beta, eps = cfg["dims"], cfg["beta"], cfg["eps"]
+    V = dims[0] * dims[1] * dims[2] * dims[3]
+    rows = []
+    for nslabs, overlap in ((1, False), (args.slabs, False), (args.slabs, True)):
+        ss = slabs.SlabSet(qcd, dims, nslabs, dtype)
+        ss.start(SEED_BASE + 4, cfg["sigma"])
+        ss.leapfrog_single_pass(beta, eps, 4, overlap=overlap)  # warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        e0.record()
+        ss.leapfrog_single_pass(beta, eps, args.steps, overlap=overlap)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        rows.append({"slabs": nslabs, "boundary_first": overlap, "ms_per_step": ms, "site_updates_per_s": V / (ms * 1e-3)})
+        del ss
+    print(json.dumps({"slab_steps": rows, "config": {"workload": f"{cfg['name']} {args.dtype} leapfrog of single-pass "
+                      f"steps with in-kernel halo push, all slabs in one process on one GPU, {args.steps} steps + the "
+                      "closing half kick"}}), flush=True)
+
+
 def run_per_kernel(args, cfg):
     """each kernel alone on ALL / EVEN / ODD with an L2 flush between timed launches (config 3's U + P is about the
     size of L2); one JSON line with a list of rows"""
@@ -480,6 +514,9 @@ def main():
                     help="length of the second timed loop that reports the power-capped regime (0: skip)")
     ap.add_argument("--peaks", action="store_true",
                     help="measure the FMA / L1 / shared-memory / L2 denominators with the library's probe kernels")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="instead of the MD-step line: the step on the lattice cut into this many slabs of timeslices in one "
+                         "process (in-kernel halo push), against the undecomposed step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-kernel", action="store_true",
                     help="instead of the MD-step line: every kernel alone on ALL/EVEN/ODD with an L2 flush between "
@@ -494,6 +531,8 @@ def main():
         run_reference(args, cfg)
     elif args.peaks:
         run_peaks(args)
+    elif args.slabs > 0:
+        run_slabs(args, cfg)
     elif args.per_kernel:
         run_per_kernel(args, cfg)
     else:

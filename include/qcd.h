@@ -338,6 +338,16 @@ int qcd_lattice_view_t(const qcd_lattice *lat, int t0, int t1, qcd_lattice **out
 int qcd_lattice_dims(const qcd_lattice *lat, int dims[4], int interior_t[2]);
 int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, const qcd_lattice *dst_lat, void *dst,
                         int dst_t, int nt, int prec, int ncomp, unsigned mu_mask, void *stream);
+/* The single-pass MD step fused with the halo transport: as qcd_md_step_single_pass on the interior timeslices of the
+ * slab lattice (or view) `lat` — P <- P + eps_p F(U_in), U_out <- reunit(exp(i eps_u P) U_in) — and the new links of
+ * the slab's first interior timeslice are ALSO stored into the upper halo of the lower neighbour's OUTPUT field
+ * lo_U_out (links mu = 0..2), those of its last interior timeslice into the lower halo of hi_U_out (all four), by the
+ * thread that computed them (peer-GPU pointers allowed; a neighbour may be NULL or this slab itself).  After all slabs
+ * have made the call the output fields are complete, halos included, and become the next step's input: no separate
+ * exchange.  Same checks as qcd_md_step_single_pass and qcd_link_update_push. */
+int qcd_md_step_single_pass_push(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
+                                 const void *U_in, void *P, void *U_out, const qcd_lattice *lo_lat, void *lo_U_out,
+                                 const qcd_lattice *hi_lat, void *hi_U_out, void *stream);
 /* Link update fused with the halo transport (SURVEY.md 8(e) "peer stores"): on the interior timeslices
  * [t0, t1) of the slab lattice (or view) `lat`, U <- exp(i eps P) U, reunitarised if reunit != 0 [O8, O9], all four
  * links of every site; the new links of the slab's first interior timeslice (te = 1) are ALSO stored into the upper

@@ -31,6 +31,7 @@ SIGNATURES = {
     "qcd_lattice_dims": (_i, [_vp, C.POINTER(C.c_int * 4), C.POINTER(C.c_int * 2)]),
     "qcd_copy_timeslices": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, _i, _i, C.c_uint, _vp]),
     "qcd_link_update_push": (_i, [_vp, _i, _d, _vp, _vp, _i, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_md_step_single_pass_push": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "qcd_lattice_destroy": (_i, [_vp]),
     "qcd_lattice_volume": (C.c_int64, [_vp]),
     "qcd_field_bytes": (_sz, [_vp, _i, _i]),
@@ -362,6 +363,13 @@ def qcd_md_host(lat, U_host, P_host, beta, eps, nsteps, device_work, stream=None
 def qcd_copy_timeslices(src_lat, src, src_t, dst_lat, dst, dst_t, nt, ncomp=72, mu_mask=0xF, stream=None):
     _check(lib.qcd_copy_timeslices(src_lat.handle, _ptr(src), src_t, dst_lat.handle, _ptr(dst), dst_t, nt, _prec(src),
                                    ncomp, mu_mask, _stream(stream)))
+
+
+def qcd_md_step_single_pass_push(lat, U_in, P, U_out, beta, eps_p, eps_u, lo_lat, lo_U_out, hi_lat, hi_U_out,
+                                 stream=None):
+    _check(lib.qcd_md_step_single_pass_push(lat.handle, _prec(U_in), beta, eps_p, eps_u, _ptr(U_in), _ptr(P),
+                                            _ptr(U_out), None if lo_lat is None else lo_lat.handle, _ptr(lo_U_out),
+                                            None if hi_lat is None else hi_lat.handle, _ptr(hi_U_out), _stream(stream)))
 
 
 def qcd_link_update_push(lat, P, U, eps, reunit, lo_lat, lo_U, hi_lat, hi_U, stream=None):

@@ -658,17 +658,12 @@ int qcd_copy_timeslices(const qcd_lattice *src_lat, const void *src, int src_t, 
                                   (cudaStream_t)stream);
 }
 
-int qcd_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
-                         const qcd_lattice *lo_lat, void *lo_U, const qcd_lattice *hi_lat, void *hi_U, void *stream) {
-    const char *fn = "qcd_link_update_push";
-    QCD_TRY(check_common(lat, prec, fn));
-    QCD_TRY(check_ptr(P, fn));
-    QCD_TRY(check_ptr(U, fn));
-    QCD_TRY(check_alias(P, U, qcd_field_bytes(lat, prec, 72), fn));
+// neighbours of a slab for the calls that store into their halos: both or neither of (lattice, field), a slab lattice
+// with the same spatial extents
+static int check_push_neighbours(const qcd_lattice *lat, int prec, const qcd_lattice *const nb[2], void *const nbU[2],
+                                 const void *P, const char *fn) {
     if (lat->p.L[3] < 3 || lat->p.t0 < 1 || lat->p.t1 > lat->p.L[3] - 1)
         return bad(QCD_EINVAL, "%s: needs a slab lattice (halo timeslices on both sides) or a view of one", fn);
-    const qcd_lattice *nb[2] = {lo_lat, hi_lat};
-    void *nbU[2] = {lo_U, hi_U};
     for (int k = 0; k < 2; k++) {
         if ((nb[k] == nullptr) != (nbU[k] == nullptr)) return bad(QCD_EINVAL, "%s: a neighbour needs both its lattice and its field", fn);
         if (!nb[k]) continue;
@@ -679,6 +674,40 @@ int qcd_link_update_push(const qcd_lattice *lat, int prec, double eps, const voi
             if (nb[k]->p.L[d] != lat->p.L[d]) return bad(QCD_EDIMS, "%s: a neighbour differs in a spatial extent", fn);
         if (nbU[k] == P) return bad(QCD_EALIAS, "%s: a neighbour's gauge field is this slab's momentum field", fn);
     }
+    return QCD_OK;
+}
+
+int qcd_md_step_single_pass_push(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u,
+                                 const void *U_in, void *P, void *U_out, const qcd_lattice *lo_lat, void *lo_U_out,
+                                 const qcd_lattice *hi_lat, void *hi_U_out, void *stream) {
+    const char *fn = "qcd_md_step_single_pass_push";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U_in, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U_out, fn));
+    const size_t fb = qcd_field_bytes(lat, prec, 72);
+    QCD_TRY(check_alias(U_in, P, fb, fn));
+    QCD_TRY(check_alias(U_in, U_out, fb, fn));
+    QCD_TRY(check_alias(P, U_out, fb, fn));
+    const qcd_lattice *nb[2] = {lo_lat, hi_lat};
+    void *nbU[2] = {lo_U_out, hi_U_out};
+    QCD_TRY(check_push_neighbours(lat, prec, nb, nbU, P, fn));
+    for (int k = 0; k < 2; k++)
+        if (nbU[k] == U_in) return bad(QCD_EALIAS, "%s: a neighbour's output field is this slab's input field", fn);
+    return launch_md_single_push(lat, prec, beta, eps_p, eps_u, U_in, P, U_out, lo_lat, lo_U_out, hi_lat, hi_U_out,
+                                 (cudaStream_t)stream);
+}
+
+int qcd_link_update_push(const qcd_lattice *lat, int prec, double eps, const void *P, void *U, int reunit,
+                         const qcd_lattice *lo_lat, void *lo_U, const qcd_lattice *hi_lat, void *hi_U, void *stream) {
+    const char *fn = "qcd_link_update_push";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(P, fn));
+    QCD_TRY(check_ptr(U, fn));
+    QCD_TRY(check_alias(P, U, qcd_field_bytes(lat, prec, 72), fn));
+    const qcd_lattice *nb[2] = {lo_lat, hi_lat};
+    void *nbU[2] = {lo_U, hi_U};
+    QCD_TRY(check_push_neighbours(lat, prec, nb, nbU, P, fn));
     return launch_link_update_push(lat, prec, eps, P, U, reunit ? 1 : 0, lo_lat, lo_U, hi_lat, hi_U, (cudaStream_t)stream);
 }
 

@@ -145,11 +145,23 @@ __device__ __forceinline__ double block_sum_warps(double v, double *buf) {
     return r;
 }
 
+// Halo transport from inside the single-pass step on a slab lattice (SURVEY.md 8(e) "peer stores"):
+// where the new links of the slab's first / last interior timeslice also go — the upper halo of the lower
+// neighbour's output field (spatial links) and the lower halo of the upper neighbour's (all four).  Pointers may be
+// peer-GPU memory; NULL: no neighbour on that side.
+struct PushP {
+    void *lo_U, *hi_U;
+    int lo_Vh, lo_L3, hi_Vh;
+};
+
 // the momentum update, the sums and the link update that follow the force of one direction (shared by both kernels)
-template <typename T, bool FUSED, bool EARLYP, bool LINK, bool SUMS>
+// PUSH: cb_lo / cb_hi = this site's checkerboard index in the neighbour's halo, or -1 (most sites)
+template <typename T, bool FUSED, bool EARLYP, bool LINK, bool SUMS, bool PUSH = false>
 __device__ __forceinline__ void finish_direction(const M3<T> &F, const M3<T> &Pm, const M3<T> &Um, const T eps,
                                                  const T eps_u, pair_t<T> *__restrict__ out,
-                                                 pair_t<T> *__restrict__ Uout, int V, int mu, int cb, double &sumK) {
+                                                 pair_t<T> *__restrict__ Uout, int V, int mu, int cb, double &sumK,
+                                                 pair_t<T> *lo_U = nullptr, int cb_lo = -1, pair_t<T> *hi_U = nullptr,
+                                                 int cb_hi = -1) {
     if (FUSED) {
         M3<T> P;
         if (EARLYP) P = Pm;
@@ -172,6 +184,10 @@ __device__ __forceinline__ void finish_direction(const M3<T> &F, const M3<T> &Pm
             mul_top2(R, E, Um);  // reunit rebuilds row 2
             reunit(R);
             store_link_cs(R, Uout, V, mu, cb);
+            if (PUSH) {  // the thread that has the boundary link in registers sends it
+                if (cb_lo >= 0 && mu < 3) store_link_cs(R, lo_U, V, mu, cb_lo);
+                if (cb_hi >= 0) store_link_cs(R, hi_U, V, mu, cb_hi);
+            }
         }
     } else {
         store_link_cs(F, out, V, mu, cb);
@@ -306,12 +322,13 @@ struct Pend {
 // exactly the six based at x, so a block whose tile lies in one timeslice also yields that timeslice's share,
 // R13) and K = sum |P_ij|^2 of the updated momenta as by-products (PAPER.md:26 fused as in PAPER.md:32), one fp64
 // partial pair per block.
-template <typename T, bool FUSED, bool EARLYP, bool LINK, bool ANISO, bool SUMS, bool TMEM>
+template <typename T, bool FUSED, bool EARLYP, bool LINK, bool ANISO, bool SUMS, bool TMEM, bool PUSH = false>
 // resident blocks per SM: 3 in fp64 (168 registers), 4 in fp32 (128 registers) — measured best of 2..6
 __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     force_plane_kernel(const LatP lat, const TileP tile, const T c /* beta/12 */, const T eps,
                        const pair_t<T> *__restrict__ U, pair_t<T> *__restrict__ out, const T eps_u,
-                       pair_t<T> *__restrict__ Uout, const T ws, const T wt, double *__restrict__ partial) {
+                       pair_t<T> *__restrict__ Uout, const T ws, const T wt, double *__restrict__ partial,
+                       const PushP push) {
     constexpr int TMEM_COLS = sizeof(T) == 8 ? 128 : 64;  // 4 x 18 (fp64) or 4 x 9 (fp32) words per thread
     __shared__ T pend_s[TMEM ? 1 : 4 * 9 * FORCE_NT];
     __shared__ uint32_t tmem_base;
@@ -335,6 +352,15 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
     const int V = lat.V;
     const int par = st.par;
     const int cb = cb_of(lat, st.s, par);
+    int cb_lo = -1, cb_hi = -1;
+    if (PUSH) {  // sites of the slab's first / last interior timeslice: where they sit in the neighbours' halos
+        const int sx = st.c[0] + lat.L[0] * (st.c[1] + lat.L[1] * st.c[2]), sp = st.c[0] + st.c[1] + st.c[2];
+        if (st.c[3] == 1 && push.lo_U) {
+            const int tp = push.lo_L3 - 1;
+            cb_lo = ((sp + tp) & 1) * push.lo_Vh + ((sx + lat.stride[3] * tp) >> 1);
+        }
+        if (st.c[3] == lat.L[3] - 2 && push.hi_U) cb_hi = (sp & 1) * push.hi_Vh + (sx >> 1);
+    }
     pend.zero();
 
 #pragma unroll 1
@@ -399,7 +425,8 @@ __global__ void __launch_bounds__(FORCE_NT, sizeof(T) == 8 ? 3 : 4)
             for (int j = 0; j < 9; j++) acc.v[j] += w.v[j];
         }
         force_from_ta(F, acc, c);
-        finish_direction<T, FUSED, EARLYP, LINK, SUMS>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK);
+        finish_direction<T, FUSED, EARLYP, LINK, SUMS, PUSH>(F, Pm, Um, eps, eps_u, out, Uout, V, mu, cb, sumK,
+                                                             (pair_t<T> *)push.lo_U, cb_lo, (pair_t<T> *)push.hi_U, cb_hi);
     }
     if (TMEM) {
         tmem_wait_st();
@@ -583,21 +610,34 @@ static ForceSel force_sel(const qcd_lattice *lat, int prec, int subset) {
 
 template <typename T, bool FUSED, bool LINK, bool ANISO, bool SUMS>
 static void launch_force_k(const qcd_lattice *lat, const ForceSel &fs, T c, T eps, const pair_t<T> *U, pair_t<T> *out,
-                           T eps_u, pair_t<T> *Uout, T ws, T wt, double *partial, cudaStream_t st) {
+                           T eps_u, pair_t<T> *Uout, T ws, T wt, double *partial, cudaStream_t st,
+                           const PushP *push = nullptr) {
     const TileP &tp = fs.tp;
     const int blocks = tp.nt[0] * tp.nt[1] * tp.nt[2] * tp.nt[3];
     const int threads = tp.tsp * tp.npar;
     // fp32 has the registers to hold the momenta from the start of a direction (-5 %); fp64 does not (+12 %)
     constexpr bool EARLYP = FUSED && sizeof(T) == 4;
+    const PushP none = {nullptr, nullptr, 0, 0, 0};
+    if constexpr (LINK && !ANISO && !SUMS) {
+        if (push) {  // single-pass step that also stores its boundary timeslices into the neighbours' halos
+            if (threads % 32 == 0)
+                force_plane_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS, true, true><<<blocks, threads, 0, st>>>(
+                    lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial, *push);
+            else
+                force_plane_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS, false, true><<<blocks, threads, 0, st>>>(
+                    lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial, *push);
+            return;
+        }
+    }
     if (fs.variant == QCD_FORCE_STAPLE)
         force_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS><<<blocks, threads, 0, st>>>(lat->p, tp, c, eps, U, out, eps_u,
                                                                                         Uout, ws, wt, partial);
     else if (threads % 32 == 0)  // whole warps: the pending parts live in Tensor Memory
         force_plane_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS, true><<<blocks, threads, 0, st>>>(
-            lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial);
+            lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial, none);
     else
         force_plane_kernel<T, FUSED, EARLYP, LINK, ANISO, SUMS, false><<<blocks, threads, 0, st>>>(
-            lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial);
+            lat->p, tp, c, eps, U, out, eps_u, Uout, ws, wt, partial, none);
 }
 
 template <typename T>
@@ -704,17 +744,28 @@ int launch_force_sums(const qcd_lattice *lat, int prec, double beta, double eps_
 // Single-pass MD step: P += eps_p F(U); Uout = reunit(exp(i eps_u P) U).  Subset ALL only (every link moves).
 template <typename T>
 static int launch_md_single_t(const qcd_lattice *lat, const ForceSel &fs, double beta, double eps_p, double eps_u,
-                              const void *U, void *P, void *Uout, cudaStream_t st) {
+                              const void *U, void *P, void *Uout, cudaStream_t st, const PushP *push) {
     launch_force_k<T, true, true, false, false>(lat, fs, (T)(beta / 12.0), (T)eps_p, (const pair_t<T> *)U,
-                                                (pair_t<T> *)P, (T)eps_u, (pair_t<T> *)Uout, T(0), T(0), nullptr, st);
-    return check_launch("md_step_single_pass");
+                                                (pair_t<T> *)P, (T)eps_u, (pair_t<T> *)Uout, T(0), T(0), nullptr, st,
+                                                push);
+    return check_launch(push ? "md_step_single_pass_push" : "md_step_single_pass");
 }
 
 int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
                      void *Uout, cudaStream_t st) {
     const ForceSel fs = force_sel(lat, prec, QCD_ALL);
-    return prec == QCD_F64 ? launch_md_single_t<double>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st)
-                           : launch_md_single_t<float>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st);
+    return prec == QCD_F64 ? launch_md_single_t<double>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st, nullptr)
+                           : launch_md_single_t<float>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st, nullptr);
+}
+
+// the same on a slab lattice, storing the new links of its boundary timeslices into the neighbours' output fields too
+int launch_md_single_push(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U,
+                          void *P, void *Uout, const qcd_lattice *lo, void *lo_U, const qcd_lattice *hi, void *hi_U,
+                          cudaStream_t st) {
+    const ForceSel fs = force_sel(lat, prec, QCD_ALL);
+    const PushP push = {lo_U, hi_U, lo ? lo->p.Vh : 0, lo ? lo->p.L[3] : 0, hi ? hi->p.Vh : 0};
+    return prec == QCD_F64 ? launch_md_single_t<double>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st, &push)
+                           : launch_md_single_t<float>(lat, fs, beta, eps_p, eps_u, U, P, Uout, st, &push);
 }
 
 }  // namespace qcd

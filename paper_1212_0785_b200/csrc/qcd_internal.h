@@ -82,6 +82,9 @@ int launch_plaquette_st(const qcd_lattice *lat, int prec, const void *U, double 
 // single-pass MD step (force.cu): P += eps_p F(U); Uout = reunit(exp(i eps_u P) U); U and Uout distinct
 int launch_md_single(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U, void *P,
                      void *Uout, cudaStream_t st);
+int launch_md_single_push(const qcd_lattice *lat, int prec, double beta, double eps_p, double eps_u, const void *U,
+                          void *P, void *Uout, const qcd_lattice *lo, void *lo_U, const qcd_lattice *hi, void *hi_U,
+                          cudaStream_t st);
 // default block tile of the stencil kernels (force.cu), computed once per lattice
 void default_force_tile(const LatP &lat, int npar, int out[4]);
 // copy `nt` timeslices starting at src_t of a pair-layout field with nc units per site into dst (same spatial

@@ -224,6 +224,28 @@ class SlabSet:
                     self.qcd.qcd_link_update(s.lat, s.P, s.U, eps, reunit=True)
                 self.kick(beta, e, overlap)
 
+    def leapfrog_single_pass(self, beta, eps, nsteps, overlap=False):
+        """the leapfrog of single-pass steps (qcd_leapfrog_single_pass regrouping) on every slab, the halo transport
+        done by the step kernel itself (qcd_md_step_single_pass_push): each step reads a slab's field with valid halos
+        and writes the second field of the slab and, for the boundary timeslices, of its neighbours.  overlap = True:
+        the boundary timeslices are launched first, so their stores travel while the inner timeslices are computed"""
+        qcd, n = self.qcd, len(self.slabs)
+        cur = [s.U for s in self.slabs]
+        oth = [s.lat.new_matrix_field(s.dtype) for s in self.slabs]
+        split = overlap and all(s.inner is not None for s in self.slabs)
+        for k in range(nsteps):
+            for which in range(3 if split else 1):
+                for r, s in enumerate(self.slabs):
+                    up, lo = (r + 1) % n, (r - 1) % n
+                    view = (list(s.edges) + [s.inner])[which] if split else s.lat
+                    qcd.qcd_md_step_single_pass_push(view, cur[r], s.P, oth[r], beta, 0.5 * eps if k == 0 else eps, eps,
+                                                     self.slabs[lo].lat, oth[lo], self.slabs[up].lat, oth[up])
+            cur, oth = oth, cur
+        for r, s in enumerate(self.slabs):
+            qcd.qcd_force_mom_update(s.lat, cur[r], s.P, beta, 0.5 * eps)
+            if cur[r] is not s.U:
+                s.U.copy_(cur[r])
+
     def gather(self, which):
         """interior timeslices of every slab as one canonical host array [V,4,3,3] of the global lattice"""
         import numpy as np

@@ -106,6 +106,35 @@ def test_slab_trajectory_equals_the_whole_lattice(qcd, orc_omp, dims, nslabs, pr
     assert abs(out[0].item() - rper_t[s.t_begin: s.t_begin + s.n].mean()) < TOL[prec]
 
 
+@pytest.mark.parametrize("dims,nslabs,prec,overlap", [((8, 8, 8, 16), 2, "f64", False), ((8, 8, 8, 16), 4, "f64", True),
+                                                      ((16, 16, 16, 32), 4, "f64", True), ((16, 16, 16, 32), 2, "f32", True),
+                                                      ((8, 8, 8, 16), 1, "f64", False), ((4, 6, 2, 8), 2, "f64", True),
+                                                      ((8, 8, 8, 16), 3, "f64", True), ((32, 8, 8, 16), 2, "f64", True)])
+@pytest.mark.parametrize("nsteps", [1, 4])
+def test_slab_single_pass_trajectory_with_in_kernel_halo_push(qcd, orc_omp, dims, nslabs, prec, overlap, nsteps):
+    """the single-pass step on slabs, halos written by the step kernel of the neighbouring slab
+    (qcd_md_step_single_pass_push): bit-identical to qcd_leapfrog_single_pass on the undecomposed lattice and within
+    tolerance of the oracle; odd and even step counts (the ping-pong ends in either buffer)"""
+    import torch
+    from paper_1212_0785_b200 import slabs
+    beta, eps, seed = 5.8, 0.05, 0x1212078500000002
+    dt = tdtype(prec)
+    full = qcd.Lattice(dims)
+    fU, fP, fW = full.new_matrix_field(dt), full.new_matrix_field(dt), full.new_matrix_field(dt)
+    qcd.qcd_hot_start(full, fU, seed, 0.5)
+    qcd.qcd_mom_refresh(full, fP, seed)
+    U0, P0 = host(qcd, full, fU), host(qcd, full, fP)
+    qcd.qcd_leapfrog_single_pass(full, fU, fP, fW, beta, eps, nsteps)
+    ss = slabs.SlabSet(qcd, dims, nslabs, dt)
+    ss.start(seed, 0.5)
+    ss.leapfrog_single_pass(beta, eps, nsteps, overlap=overlap)
+    torch.cuda.synchronize()
+    gU, gP = ss.gather("U"), ss.gather("P")
+    assert np.array_equal(gU, host(qcd, full, fU)) and np.array_equal(gP, host(qcd, full, fP))
+    rU, rP = orc_omp.leapfrog(dims, beta, eps, nsteps, U0, P0)
+    assert rel(gU, rU) < TOL[prec] and rel(gP, rP) < TOL[prec]
+
+
 def test_link_update_push_arguments_and_halo_only_stores(qcd):
     """argument checks before anything is enqueued; the push writes the neighbours' halos and nothing else of them,
     and leaves the slab's own halos alone"""
