@@ -213,7 +213,7 @@ def run_ours(args, cfg):
     prec = qcd.F64 if args.dtype == "f64" else qcd.F32
     fma_peak = qcd.probe_rate(qcd.PROBE_FMA, prec)
     fma_src = "measured in this run: qcd_probe_launch(QCD_PROBE_FMA), best of 3, CUDA events"
-    time.sleep(0.5)  # let the board cool off the probe before the timed region
+    time.sleep(2.0)  # let the board cool off the probe (full-power FMA for 0.1 s) before the timed region
 
     nwarm = args.warmup + (args.warmup & 1 if single else 0)  # even, so the timed steps start from bufs[0]
     for k in range(nwarm):
