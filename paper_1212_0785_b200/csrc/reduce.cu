@@ -29,7 +29,7 @@ __device__ __forceinline__ double block_sum(double v) {
 
 // ---- per-site values -----------------------------------------------------------------------
 
-// sum_{mu<nu} Re tr P_mu_nu(x), P_mu_nu(x) = [U_mu(x) U_nu(x+mu)] [U_nu(x) U_mu(x+nu)]^dagger
+// sum_{mu<nu} Re tr P_mu_nu(x), P_mu_nu(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger
 // which: 0 = all six planes, 1 = the three space-space planes, 2 = the three space-time planes (R19)
 template <typename T>
 __device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T> *__restrict__ U, int cb,
@@ -47,14 +47,15 @@ __device__ __forceinline__ double site_plaquette(const LatP &lat, const pair_t<T
 #pragma unroll
         for (int nu = mu + 1; nu < 4; nu++) {
             if ((which == 1 && nu == 3) || (which == 2 && nu != 3)) continue;
-            M3<T> A, X, Y;
+            // Re tr{[U_mu(x) U_nu(x+mu)] U_mu(x+nu)^dag U_nu(x)^dag}, left to right: three matrices besides U_mu(x) are
+            // live at a time (the two-bracket form needs four and spilled at 168 registers)
+            M3<T> A, X, Z;
             load_link(A, U, V, nu, cbf[mu]);
             mul<false, false, false>(X, Um, A);
-            M3<T> B;
+            load_link(A, U, V, mu, cbf[nu]);
+            mul<false, true, false>(Z, X, A);
             load_link(A, U, V, nu, cb);
-            load_link(B, U, V, mu, cbf[nu]);
-            mul<false, false, false>(Y, A, B);
-            acc += retr_mul_dag(X, Y);
+            acc += retr_mul_dag(Z, A);
         }
     }
     return (double)acc;
