@@ -207,7 +207,8 @@ int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, doub
  *   U_work scratch gauge field, qcd_field_bytes(lat, prec, 72) bytes; the final links are always left in U.
  *   workspace, workspace_bytes: at least qcd_workspace_bytes(lat), else QCD_EWORKSPACE (also returned when a tuned
  *          tile has more blocks than the workspace has room for).  All checks are made before anything is enqueued.
- * Deterministic run to run at a fixed launch configuration (one partial per block, fixed order). */
+ * Deterministic run to run at a fixed launch configuration (one partial per block and timeslice of its tile, summed in
+ * a fixed order). */
 int qcd_trajectory(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U, void *P,
                    void *U_work, double *obs, double *per_t, void *workspace, size_t workspace_bytes, void *stream);
 
