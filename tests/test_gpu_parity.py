@@ -511,6 +511,58 @@ def test_md_step_single_pass(qcd, orc_omp, prec, dims):
     assert e.value.code == qcd.EALIAS
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (12, 6, 10, 4), (32, 32, 48, 8)])
+def test_kernels_write_nothing_outside_their_fields(qcd, dims, prec):
+    """every output of the step kernels sits inside a larger buffer filled with a sentinel: momenta, second gauge
+    field, workspace, observables, and the neighbours' fields of the calls that push halos.  After the calls the
+    guard bands are untouched (whole warps, partial warps, the z-blocked launch order)"""
+    import torch
+    dt = tdtype(prec)
+    G, SENT = 4096, -7.25
+
+    def guarded(n, dtype):
+        base = torch.full((n + 2 * G,), SENT, dtype=dtype, device="cuda")
+        return base, base[G: G + n]
+
+    def intact(base, n):
+        return bool((base[:G] == SENT).all()) and bool((base[G + n:] == SENT).all())
+
+    lat = qcd.Lattice(dims)
+    n = lat.nchunks * 36 * 32 * 2
+    bases, f = zip(*(guarded(n, dt) for _ in range(3)))
+    U, P, W = (x.view(lat.nchunks, 36, 32, 2) for x in f)
+    qcd.qcd_hot_start(lat, U, 11, 0.4)
+    qcd.qcd_mom_refresh(lat, P, 12)
+    nws = lat.workspace_bytes() // 8
+    wsb, ws = guarded(nws, torch.float64)
+    obb, obs = guarded(2 * 3, torch.float64)
+    ptb, per_t = guarded(3 * dims[3], torch.float64)
+    qcd.qcd_md_step_single_pass(lat, U, P, W, 5.8, 0.03, 0.03)
+    qcd.qcd_force_mom_update(lat, W, P, 5.8, 0.03)
+    qcd.qcd_link_update(lat, P, W, 0.03, reunit=True)
+    qcd.qcd_trajectory(lat, U, P, W, 5.8, 0.03, 2, obs.view(3, 2), per_t.view(3, dims[3]), ws)
+    qcd.qcd_plaquette(lat, U, obs[0:1], per_t[: dims[3]], ws)
+    torch.cuda.synchronize()
+    assert all(intact(b, n) for b in bases) and intact(wsb, nws) and intact(obb, 6) and intact(ptb, 3 * dims[3])
+    assert bool(torch.isfinite(U).all()) and bool(torch.isfinite(P).all())
+    if dims[3] % 4 == 0 and dims[3] >= 8:  # two slabs, halos pushed by the kernels
+        half = dims[3] // 2
+        a, b = qcd.Lattice(dims, slab=(0, half)), qcd.Lattice(dims, slab=(half, half))
+        m = a.nchunks * 36 * 32 * 2
+        sb, sf = zip(*(guarded(m, dt) for _ in range(6)))
+        Ua, Pa, Wa, Ub, Pb, Wb = (x.view(a.nchunks, 36, 32, 2) for x in sf)
+        for L, Uf, Pf in ((a, Ua, Pa), (b, Ub, Pb)):
+            qcd.qcd_hot_start(L, Uf, 11, 0.4)
+            qcd.qcd_mom_refresh(L, Pf, 12)
+        qcd.qcd_md_step_single_pass_push(a, Ua, Pa, Wa, 5.8, 0.03, 0.03, b, Wb, b, Wb)
+        qcd.qcd_md_step_single_pass_push(b, Ub, Pb, Wb, 5.8, 0.03, 0.03, a, Wa, a, Wa)
+        qcd.qcd_link_update_push(a, Pa, Wa, 0.03, True, b, Wb, b, Wb)
+        qcd.qcd_link_update_push(b, Pb, Wb, 0.03, True, a, Wa, a, Wa)
+        torch.cuda.synchronize()
+        assert all(intact(x, m) for x in sb)
+
+
 def test_z_blocked_launch_order_whole_field(qcd, orc_omp):
     """32x32x48x8 fp64: three timeslices of U are 85 MB, above the threshold at which the plane kernel launches its
     blocks z-block by z-block (force.cu: canonical_block, two z-blocks of 24 planes here).  Whole-field comparison of
