@@ -36,7 +36,8 @@
  * OWNERSHIP AND ASYNCHRONY
  *   Unless a parameter says "host", every pointer is a DEVICE pointer owned by the caller (e.g. a
  *   PyTorch tensor's data_ptr()).  The library allocates no device memory: fields, outputs and
- *   workspace are the caller's and must stay alive until the stream work has completed.  `stream`
+ *   workspace are the caller's and must stay alive until the stream work has completed (the library image
+ *   itself carries one fixed 256 KiB device array, the scratch of qcd_plaquette_noalloc).  `stream`
  *   is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call only enqueues
  *   work on `stream` and returns without synchronising; reduction results are written to device
  *   doubles.  qcd_lattice is host-only, immutable after creation and may be shared across threads.
@@ -144,6 +145,31 @@ int qcd_mom_refresh(const qcd_lattice *lat, int prec, int subset, uint64_t seed,
  * out_avg, out_per_t: device doubles.  workspace: qcd_workspace_bytes(lat) device bytes. */
 int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
                   void *workspace, void *stream);
+
+/* qcd_plaquette without a workspace argument, for callers that cannot obtain device memory.  Two kinds of caller
+ * are meant: code running inside an application whose memory manager has taken the whole device for its own pool
+ * (the framework's allocator serves every package and a measurement routine called from inside
+ * holds no handle to it, so a cudaMalloc of its own fails or competes with the pool), and code that measures inside
+ * a running trajectory, where cudaMalloc / cudaFree would make every stream of the device wait.  The caller still
+ * passes U and the outputs; the first-pass partial sums, which qcd_plaquette keeps in `workspace`, go to an array
+ * that is part of the library itself.  Same kernels, same reduction order and same results as qcd_plaquette [O6].
+ *   LIMIT    the array holds 32768 doubles (256 KiB of device memory on every GPU the library is loaded on, from
+ *            load until the process exits).  A lattice needs 2 Lt ceil(Lx Ly Lz / 2048) of them: all five BASELINE
+ *            lattices fit (48^3 x 96 needs 10368), 64^3 x 128 just fits; anything larger returns QCD_EWORKSPACE with
+ *            the two numbers in qcd_last_error() and enqueues nothing — use qcd_plaquette there.
+ *   SET-UP   the first call on each device (with that device current) asks the CUDA runtime once for the array's
+ *            device address and keeps it; make that first call outside any stream capture.  Later calls only launch.
+ *   ALLOCATION  none: neither this call nor anything below it calls cudaMalloc, cudaFree or an allocating library
+ *            routine.
+ *   SHARING  all calls on one device use the same array, and it keeps whatever the last call left there.  Nothing
+ *            has to be cleared — the first pass rewrites every slot the second pass reads — but two calls whose
+ *            kernels can run at the same time on one GPU (different streams without an ordering between them,
+ *            different host threads) overwrite each other's partial sums and return garbage: order them, e.g. by
+ *            using one stream.  Calls on different GPUs do not interfere.
+ * Other errors as qcd_plaquette (QCD_EINVAL for a NULL lattice, U or out_avg; QCD_EALIGN); QCD_ECUDA if the address
+ * query or a launch fails, QCD_EINVAL on a device ordinal >= 64. */
+int qcd_plaquette_noalloc(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                          void *stream);
 
 /* Global / subset sum [O12] ("sum") of a per-site quantity of `field`:
  *   QCD_SUM_SCALAR  real field (QCD_LAYOUT_REAL) with ncomp components: out[c] = sum_x field_c(x), c < ncomp <= 64

@@ -46,6 +46,7 @@ SIGNATURES = {
     "qcd_reunit": (_i, [_vp, _i, _i, _vp, _vp]),
     "qcd_mom_refresh": (_i, [_vp, _i, _i, _u64, _u32, _vp, _vp]),
     "qcd_plaquette": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp]),
+    "qcd_plaquette_noalloc": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "qcd_sum": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "qcd_sum_multi": (_i, [_vp, _i, _i, _i, _vp, _vp, _i, _vp, _vp, _vp]),
     "qcd_md_step": (_i, [_vp, _i, _d, _d, _d, _vp, _vp, _vp]),
@@ -232,6 +233,14 @@ def qcd_mom_refresh(lat, P, seed, stream_id=0, subset=ALL, stream=None):
 def qcd_plaquette(lat, U, out_avg, out_per_t, workspace, stream=None):
     _check(lib.qcd_plaquette(lat.handle, _prec(U), _ptr(U), _ptr(out_avg), _ptr(out_per_t), _ptr(workspace),
                              _stream(stream)))
+
+
+def qcd_plaquette_noalloc(lat, U, out_avg, out_per_t, stream=None):
+    """qcd_plaquette for a caller that cannot get device memory for a workspace (a routine inside an application
+    whose memory manager owns the whole device, or one that must not stall a running trajectory with cudaMalloc):
+    the partial sums use the 256 KiB array built into the library.  Lattices that need more than 32768 partial
+    sums raise QcdError(EWORKSPACE); calls that overlap on one GPU race on that array (include/qcd.h)."""
+    _check(lib.qcd_plaquette_noalloc(lat.handle, _prec(U), _ptr(U), _ptr(out_avg), _ptr(out_per_t), _stream(stream)))
 
 
 def qcd_sum(lat, kind, ncomp, field, out, workspace, subset=ALL, stream=None):

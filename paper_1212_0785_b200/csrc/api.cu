@@ -251,6 +251,25 @@ int qcd_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_a
     return launch_plaquette(lat, prec, U, out_avg, out_per_t, (double *)workspace, (cudaStream_t)stream);
 }
 
+// qcd_plaquette for callers that have no device memory to offer as workspace (include/qcd.h): the partial sums
+// go to the array built into the library (reduce.cu).  No allocation here or below; the size is checked before
+// any CUDA call.
+int qcd_plaquette_noalloc(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                          void *stream) {
+    const char *fn = "qcd_plaquette_noalloc";
+    QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_ptr(U, fn));
+    if (!out_avg) return bad(QCD_EINVAL, "%s: NULL output", fn);
+    const long long need = (long long)lat->red_nseg * lat->red_chunks_per_seg;
+    if (need > NOALLOC_MAX_PARTIALS) {
+        set_error("%s: this lattice needs %lld partial sums, the built-in scratch holds %d (2 Lt ceil(Lx Ly Lz / 2048) "
+                  "must not exceed it); use qcd_plaquette with a workspace of your own",
+                  fn, need, NOALLOC_MAX_PARTIALS);
+        return QCD_EWORKSPACE;
+    }
+    return launch_plaquette_noalloc(lat, prec, U, out_avg, out_per_t, (cudaStream_t)stream);
+}
+
 static int check_sum_args(int kind, int ncomp, const char *fn) {
     if (kind != QCD_SUM_SCALAR && kind != QCD_SUM_NORM2 && kind != QCD_SUM_RETR) return bad(QCD_EINVAL, "%s: unknown kind", fn);
     if (ncomp < 1) return bad(QCD_EINVAL, "%s: ncomp < 1", fn);

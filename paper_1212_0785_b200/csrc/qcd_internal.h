@@ -41,6 +41,9 @@ constexpr int RED_CHUNK = 1024;    // sites per first-pass block
 constexpr int RED_GENERIC_CHUNKS = 256;  // first-pass blocks per subset on the subset_id path
 constexpr int MAX_NSUB = 4096;
 constexpr int MAX_SUM_NCOMP = 64;
+// qcd_plaquette_noalloc: first-pass partial sums that fit the library's built-in scratch array (reduce.cu);
+// 32768 doubles = 256 KiB of device memory per GPU, held from the moment the library is loaded there until exit
+constexpr int NOALLOC_MAX_PARTIALS = 32768;
 
 }  // namespace qcd
 
@@ -111,6 +114,10 @@ int launch_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n
                       const uint32_t *mu_j, uint32_t *words, double *uniforms, double *gauss, cudaStream_t st);
 int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
                      double *ws, cudaStream_t st);
+// qcd_plaquette_noalloc (reduce.cu): launch_plaquette with the partial sums in the library's built-in scratch array;
+// the caller has checked red_nseg * red_chunks_per_seg <= NOALLOC_MAX_PARTIALS
+int launch_plaquette_noalloc(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                             cudaStream_t st);
 int launch_sum(const qcd_lattice *lat, int prec, int subset, int kind, int ncomp, const void *field, double *out,
                double *ws, cudaStream_t st);
 int launch_sum_multi(const qcd_lattice *lat, int prec, int kind, int ncomp, const void *field,

@@ -5,6 +5,8 @@
 // Pass 1: one block per chunk, fixed per-thread order, fixed shuffle/shared tree -> one partial.
 // Pass 2: one block per result sums the partials in a fixed order.  The geometry depends only on
 // the lattice, never on tuning, so results are bit-identical from run to run.
+#include <mutex>
+
 #include "qcd_internal.h"
 #include "site.cuh"
 #include "su3.cuh"
@@ -226,6 +228,63 @@ int launch_plaquette(const qcd_lattice *lat, int prec, const void *U, double *ou
                      cudaStream_t st) {
     return prec == QCD_F64 ? plaquette_t<double>(lat, U, out_avg, out_per_t, ws, st)
                            : plaquette_t<float>(lat, U, out_avg, out_per_t, ws, st);
+}
+
+// ---- qcd_plaquette_noalloc: the same two passes with the partial sums in memory the library brings along ----
+//
+// Some callers of this library cannot hand it a workspace because they have no way to get device memory: code
+// that runs inside an application whose own memory manager has claimed the whole device (the setting of
+// PAPER.md:71,83, where every package's allocations are redirected to one pool that such a caller holds no
+// handle to), and measurement code inside a running trajectory, where a cudaMalloc / cudaFree pair would
+// stall every stream of the device.  For them the first-pass partials live in this file-scope array.  It is
+// part of the library image: every GPU on which the library is loaded carries its 256 KiB until the process
+// exits, whether or not the call is ever made.
+//
+// g_noalloc_partials names the array in DEVICE code.  In host code the same identifier is only a handle for the
+// runtime's symbol calls — it is not a device address, and a kernel handed `g_noalloc_partials` from the host
+// would write somewhere else entirely — so the launcher below asks the runtime for the array's address on the
+// current device, once per device, and passes that pointer to the kernels.
+static __device__ __align__(256) double g_noalloc_partials[NOALLOC_MAX_PARTIALS];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static double *g_noalloc_addr[NOALLOC_MAX_DEVICES];  // device address of g_noalloc_partials on device i; NULL = not asked yet
+static std::mutex g_noalloc_mutex;
+
+// the array's address on the CURRENT device (set-up on the first call per device: one cudaGetSymbolAddress)
+static int noalloc_partials(double **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        set_error("qcd_plaquette_noalloc: cudaGetDevice: %s", cudaGetErrorString(e));
+        return QCD_ECUDA;
+    }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) {
+        set_error("qcd_plaquette_noalloc: device ordinal %d outside the %d this call keeps an address for", dev,
+                  NOALLOC_MAX_DEVICES);
+        return QCD_EINVAL;
+    }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_partials);
+        if (e != cudaSuccess || !p) {
+            set_error("qcd_plaquette_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            return QCD_ECUDA;
+        }
+        g_noalloc_addr[dev] = (double *)p;
+    }
+    *out = g_noalloc_addr[dev];
+    return QCD_OK;
+}
+
+// Nothing in the array has to start at zero: pass 1 stores one partial per block into every slot pass 2 reads
+// (slots [0, nseg*cps)), so what an earlier call left behind is overwritten before it is looked at.
+int launch_plaquette_noalloc(const qcd_lattice *lat, int prec, const void *U, double *out_avg, double *out_per_t,
+                             cudaStream_t st) {
+    double *ws = nullptr;
+    const int rc = noalloc_partials(&ws);
+    if (rc != QCD_OK) return rc;
+    return launch_plaquette(lat, prec, U, out_avg, out_per_t, ws, st);
 }
 
 // out[g] = scale * sum of the `count` per-block partials partial[g*count .. (g+1)*count), g < ngroups, fixed
