@@ -351,8 +351,12 @@ int qcd_rng_blocks(uint64_t seed, uint32_t stream_id, uint32_t purpose, int n, c
  *   - qcd_force_mom_update_sums averages the plaquette over the interior sites and sums K over them; the
  *     reductions with per-timeslice outputs (qcd_plaquette out_per_t, qcd_sum_multi, qcd_inner_product_multi)
  *     return t_count + 2 values of which the interior ones are the global lattice's; ranks are combined in fixed
- *     rank order by the caller (paper_1212_0785_b200/slabs.py).  qcd_trajectory and the by-product per-timeslice
- *     sums need the whole lattice.
+ *     rank order by the caller (paper_1212_0785_b200/slabs.py).  The by-product per-timeslice sums need the whole
+ *     lattice;
+ *   - the calls that make several link updates in a row (qcd_leapfrog, qcd_leapfrog_energy, qcd_leapfrog_single_pass,
+ *     qcd_trajectory, qcd_nested_leapfrog, qcd_md_host) return QCD_EINVAL on a slab lattice or a t-view: the halos
+ *     cannot be refreshed inside the call.  Build the trajectory from the single-step calls and the transport
+ *     (paper_1212_0785_b200/slabs.py does).
  * qcd_copy_timeslices is the transport: it copies nt timeslices of a pair-layout field (ncomp reals per site, 72 for
  * matrix fields; mu_mask selects the links of a matrix field, bit mu) between two lattices with the same spatial
  * extents; dst may be a peer GPU's memory (direct stores over NVLink).  QCD_EDIMS if the spatial extents differ. */
@@ -411,7 +415,11 @@ int qcd_probe_launch(int what, int prec, int reps, void *scratch, size_t scratch
  * so that for one step both PCIe directions are busy at once.  `stream` is joined at entry and at exit with events
  * (the work is ordered after what `stream` held and before what is enqueued on it next); the host is never
  * synchronised.  Lattices with fewer than 8 slabs run on `stream` alone.
- * device_work: qcd_md_host_work_bytes(lat, prec) device bytes. */
+ * device_work: qcd_md_host_work_bytes(lat, prec) device bytes.
+ * State the library keeps for this call (the one exception to "owns nothing" above): per host thread and device,
+ * the three internal streams and a pool of events, created by the thread's first pipelined call with that device
+ * current, reused afterwards and destroyed when the thread exits.  Two threads must not run the call on the same
+ * device_work at the same time. */
 int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host,
                 void *P_host, void *device_work, void *stream);
 

@@ -60,6 +60,14 @@ static int check_alias2(const void *a, size_t bytes_a, const void *b, size_t byt
 static int check_alias(const void *a, const void *b, size_t bytes, const char *fn) {
     return check_alias2(a, bytes, b, bytes, fn);
 }
+// The multi-step integrators run several link updates in a row and have no way to refresh halo timeslices in
+// between (and their link update on QCD_ALL would advance the halos with stale momenta), so on a slab lattice or
+// a t-view they would return wrong fields without saying so: whole lattices only.
+static int check_whole(const qcd_lattice *lat, const char *fn) {
+    if (lat->p.t0 != 0 || lat->p.t1 != lat->p.L[3] || lat->p.gV != lat->p.V)
+        return bad(QCD_EINVAL, "%s: needs the whole lattice, not a slab lattice or a t-view (halos cannot be refreshed inside the call)", fn);
+    return QCD_OK;
+}
 // the kernels index the units of a field with 32 bits: nc units per site need nc (V + 32) < 2^32
 static int check_units(const qcd_lattice *lat, long long nc, const char *fn) {
     if (nc * ((long long)lat->p.V + 32) >= (1ll << 32)) return bad(QCD_EDIMS, "%s: units per site x V must be < 2^32", fn);
@@ -323,6 +331,7 @@ int qcd_leapfrog(const qcd_lattice *lat, int prec, double beta, double eps, int 
                  void *stream) {
     const char *fn = "qcd_leapfrog";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
@@ -352,6 +361,7 @@ int qcd_leapfrog_energy(const qcd_lattice *lat, int prec, double beta, double ep
                         double *out, void *workspace, void *stream) {
     const char *fn = "qcd_leapfrog_energy";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
@@ -384,6 +394,7 @@ int qcd_leapfrog_single_pass(const qcd_lattice *lat, int prec, double beta, doub
                              void *P, void *U_work, void *stream) {
     const char *fn = "qcd_leapfrog_single_pass";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_ptr(U_work, fn));
@@ -414,6 +425,7 @@ int qcd_trajectory(const qcd_lattice *lat, int prec, double beta, double eps, in
                    double *obs, double *per_t, void *workspace, size_t workspace_bytes, void *stream) {
     const char *fn = "qcd_trajectory";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_ptr(U_work, fn));
@@ -495,6 +507,7 @@ int qcd_nested_leapfrog(const qcd_lattice *lat, int prec, const double beta_s[2]
                         int n_outer, int n_inner, void *U, void *P, void *stream) {
     const char *fn = "qcd_nested_leapfrog";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     QCD_TRY(check_ptr(U, fn));
     QCD_TRY(check_ptr(P, fn));
     QCD_TRY(check_alias(U, P, qcd_field_bytes(lat, prec, 72), fn));
@@ -753,6 +766,7 @@ int qcd_md_host(const qcd_lattice *lat, int prec, double beta, double eps, int n
                 void *device_work, void *stream) {
     const char *fn = "qcd_md_host";
     QCD_TRY(check_common(lat, prec, fn));
+    QCD_TRY(check_whole(lat, fn));
     if (!U_host || !P_host) return bad(QCD_EINVAL, "%s: NULL host buffer", fn);
     QCD_TRY(check_ptr(device_work, fn));
     if (nsteps < 0) return bad(QCD_EINVAL, "%s: nsteps < 0", fn);

@@ -93,6 +93,29 @@ def test_argument_validation_happens_before_any_cuda_call(qcd):
     assert L.qcd_md_host(h, qcd.F64, 5.0, 0.1, 1, None, a, b, None) == qcd.EINVAL
 
 
+def test_multi_step_integrators_refuse_slab_lattices_and_views(qcd):
+    """several link updates in one call cannot refresh halos in between: QCD_EINVAL before anything is enqueued"""
+    L = qcd.lib
+    full = qcd.Lattice((4, 4, 4, 8))
+    slab = qcd.Lattice((4, 4, 4, 8), slab=(2, 4))
+    view = full.view_t(2, 6)
+    fb = full.field_bytes(qcd.F64)
+    a, b, c, o = 0x10000000, 0x10000000 + 2 * fb, 0x10000000 + 4 * fb, 0x10000000 + 6 * fb
+    two = (C.c_double * 2)(5.0, 1.0)
+    for lat in (slab, view):
+        h = lat.handle
+        assert L.qcd_leapfrog(h, qcd.F64, 5.0, 0.1, 2, a, b, None) == qcd.EINVAL
+        assert b"whole lattice" in L.qcd_last_error()
+        assert L.qcd_leapfrog(h, qcd.F64, 5.0, 0.1, 1, a, b, None) == qcd.EINVAL
+        assert L.qcd_leapfrog_energy(h, qcd.F64, 5.0, 0.1, 2, a, b, o, o, None) == qcd.EINVAL
+        assert L.qcd_leapfrog_single_pass(h, qcd.F64, 5.0, 0.1, 2, a, b, c, None) == qcd.EINVAL
+        assert L.qcd_trajectory(h, qcd.F64, 5.0, 0.1, 2, a, b, c, o, None, o, 1 << 30, None) == qcd.EINVAL
+        assert L.qcd_nested_leapfrog(h, qcd.F64, C.byref(two), C.byref(two), 1.0, 2, 2, a, b, None) == qcd.EINVAL
+        assert L.qcd_md_host(h, qcd.F64, 5.0, 0.1, 1, a, b, c, None) == qcd.EINVAL
+    # a view that spans every timeslice is the whole lattice again: the call gets past this check (and fails the next)
+    assert L.qcd_leapfrog(full.view_t(0, 8).handle, qcd.F64, 5.0, 0.1, 2, a, a, None) == qcd.EALIAS
+
+
 def test_product_path_does_not_import_the_oracle():
     """the CUDA package must not reference oracle/ (and the oracle must not reference the package)"""
     pkg = os.path.join(ROOT, "paper_1212_0785_b200")
