@@ -89,9 +89,10 @@ struct Hops {
     unsigned wrap;   // bit d: c[d] == L[d] - 1;  bit 4 + d: c[d] == 0
     // every thread of the block calls init before the first use; the caller synchronises the block
     __device__ __forceinline__ void init(const LatP &lat, const Site &st, int *t) {
-        if (threadIdx.x < 4) {
-            t[threadIdx.x] = lat.stride[threadIdx.x];
-            t[4 + threadIdx.x] = -(lat.L[threadIdx.x] - 1) * lat.stride[threadIdx.x];
+        // strided: a tuned tile may give a block fewer than four threads (tile (2,1,1,1): two)
+        for (int d = threadIdx.x; d < 4; d += blockDim.x) {
+            t[d] = lat.stride[d];
+            t[4 + d] = -(lat.L[d] - 1) * lat.stride[d];
         }
         tab = t;
         wrap = 0;

@@ -286,12 +286,14 @@ def test_gauge_force_generic_matrices(qcd, orc, prec):
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("variant,tile", [("plane", None), ("plane", (4, 2, 2, 2)), ("plane", (8, 4, 2, 2)),
                                           ("plane", (4, 4, 4, 2)), ("plane", (2, 2, 2, 2)), ("staple", None),
-                                          ("staple", (4, 2, 2, 2)), ("staple", (8, 2, 2, 4))])
+                                          ("staple", (4, 2, 2, 2)), ("staple", (8, 2, 2, 4)),
+                                          # blocks of 1, 2 and 4 threads: fewer threads than the hop table has rows
+                                          ("plane", (2, 1, 1, 1)), ("plane", (2, 2, 1, 1)), ("staple", (2, 1, 1, 1))])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 4), (16, 8, 8, 16)])
 def test_force_kernel_variants(qcd, orc_omp, prec, variant, tile, dims):
     """both force kernels (the tuner's database is the knob: variant and 4-D block tile) against the oracle,
     fused and unfused, over several tiles, with tiles that span a whole extent (periodic wrap inside the
-    tile) and with blocks that are not a whole number of warps"""
+    tile), with blocks that are not a whole number of warps, and with blocks of one, two and four threads"""
     if tile and any(d % t for d, t in zip(dims, tile)):
         pytest.skip("tile does not divide the lattice")
     lat = qcd.Lattice(dims)
