@@ -9,6 +9,7 @@
 // so that, for a single step, both PCIe directions are busy at once and the kernels hide behind the copies.  With
 // nsteps > 1 the first step overlaps the upload, the last one the download, the steps between run on the whole
 // lattice.  The caller's stream is joined at entry and at exit with events; nothing synchronises the host.
+#include <map>
 #include <vector>
 
 #include "qcd_internal.h"
@@ -17,15 +18,26 @@ namespace qcd {
 
 namespace {
 
+// The three streams and the events belong to one device, so there is one Pipe per (host thread, device): created on
+// the first qcd_md_host call of that thread with that device current, reused by later calls, destroyed when the
+// thread exits (for the main thread: before the CUDA runtime's own exit handlers run).
 struct Pipe {
     cudaStream_t up = nullptr, comp = nullptr, down = nullptr;
     std::vector<cudaEvent_t> ev;
     size_t used = 0;
+    Pipe() = default;
+    Pipe(const Pipe &) = delete;
+    Pipe &operator=(const Pipe &) = delete;
+    ~Pipe() {
+        for (cudaEvent_t e : ev) cudaEventDestroy(e);
+        for (cudaStream_t s : {up, comp, down})
+            if (s) cudaStreamDestroy(s);
+    }
     bool ok() {
-        if (up) return true;
-        return cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking) == cudaSuccess &&
-               cudaStreamCreateWithFlags(&comp, cudaStreamNonBlocking) == cudaSuccess &&
-               cudaStreamCreateWithFlags(&down, cudaStreamNonBlocking) == cudaSuccess;
+        if (up && comp && down) return true;
+        return (up || cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking) == cudaSuccess) &&
+               (comp || cudaStreamCreateWithFlags(&comp, cudaStreamNonBlocking) == cudaSuccess) &&
+               (down || cudaStreamCreateWithFlags(&down, cudaStreamNonBlocking) == cudaSuccess);
     }
     cudaEvent_t event() {  // events are reused from call to call (recording again is legal once waited on)
         if (used == ev.size()) {
@@ -36,7 +48,7 @@ struct Pipe {
         return ev[used++];
     }
 };
-thread_local Pipe g_pipe;
+thread_local std::map<int, Pipe> g_pipes;  // key: device ordinal
 
 int cuda_rc(cudaError_t e, const char *what) {
     if (e == cudaSuccess) return QCD_OK;
@@ -67,7 +79,9 @@ bool md_host_can_pipeline(const qcd_lattice *lat) {
 // work: 4 device fields: U_a, P, U_b, staging (8 slab buffers of canonical data).  All arguments validated by the caller.
 int md_host_pipelined(const qcd_lattice *lat, int prec, double beta, double eps, int nsteps, void *U_host,
                       void *P_host, void *work, size_t fb, cudaStream_t user) {
-    Pipe &pp = g_pipe;
+    int dev = -1;
+    PIPE_TRY(cuda_rc(cudaGetDevice(&dev), "cudaGetDevice"));
+    Pipe &pp = g_pipes[dev];
     if (!pp.ok()) return cuda_rc(cudaGetLastError(), "stream creation");
     pp.used = 0;
     const int Lt = lat->p.L[3], ns = slab_count(Lt), ts = Lt / ns;
