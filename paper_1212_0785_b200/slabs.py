@@ -52,22 +52,39 @@ class SlabComm:
         self.lower, self.upper = (rank - 1) % world, (rank + 1) % world
 
     def exchange(self, to_lower, to_upper):
-        """send one face to each neighbour, receive theirs: returns (from_lower, from_upper).  Tags keep the two
-        messages apart when both neighbours are the same rank (world = 2)."""
+        """send one face to each neighbour, receive theirs: returns (from_lower, from_upper).  The two messages may
+        differ in size (the face sent down carries three links, the one sent up four).  When both neighbours are the
+        same rank (world = 2) gloo keeps the messages apart by tag; NCCL ignores tags and matches the sends and
+        receives of a pair of ranks in the order they were posted, which is why the order below is the same on both
+        sides: up-going face first (my first send, the peer's first receive), down-going face second.
+        Device tensors over a CPU-only backend (gloo: the two-processes-on-one-GPU test) are staged through host
+        memory; over NCCL they travel as they are."""
         if self.world == 1:
             return to_upper.clone(), to_lower.clone()
         d = self.dist
+        dev = to_lower.device
+        staged = self._staged(to_lower)
+        if staged:
+            to_lower, to_upper = to_lower.cpu(), to_upper.cpu()
         from_lower, from_upper = torch.empty_like(to_upper), torch.empty_like(to_lower)
         ops = [d.P2POp(d.isend, to_upper, self.upper, tag=0), d.P2POp(d.isend, to_lower, self.lower, tag=1),
                d.P2POp(d.irecv, from_lower, self.lower, tag=0), d.P2POp(d.irecv, from_upper, self.upper, tag=1)]
         for r in d.batch_isend_irecv(ops):
             r.wait()
+        if staged:
+            from_lower, from_upper = from_lower.to(dev), from_upper.to(dev)
         return from_lower, from_upper
+
+    def _staged(self, t):
+        """device tensors over a CPU-only backend go through host memory (see exchange)"""
+        return t.device.type == "cuda" and self.dist.get_backend() == "gloo"
 
     def combine(self, local):
         """all ranks' values of a small tensor, summed in rank order (one all_gather; no rank-dependent order)"""
         if self.world == 1:
             return local.clone()
+        if self._staged(local):
+            return self.combine(local.cpu()).to(local.device)
         parts = [torch.empty_like(local) for _ in range(self.world)]
         self.dist.all_gather(parts, local)
         return ordered_sum(parts)
@@ -76,6 +93,8 @@ class SlabComm:
         """per-timeslice values of every rank, concatenated in rank order = global timeslice order"""
         if self.world == 1:
             return local.clone()
+        if self._staged(local):
+            return self.gather_concat(local.cpu()).to(local.device)
         sizes = [torch.zeros(1, dtype=torch.int64, device=local.device) for _ in range(self.world)]
         self.dist.all_gather(sizes, torch.tensor([local.numel()], dtype=torch.int64, device=local.device))
         m = int(max(s.item() for s in sizes))
@@ -105,13 +124,38 @@ class _SlabOps:
         self.qcd.qcd_hot_start(self.lat, self.U, seed, sigma)
         self.qcd.qcd_mom_refresh(self.lat, self.P, seed)
 
+    # A face is one timeslice of links.  qcd_copy_timeslices moves it between the slab and timeslice 0 of `face_lat`,
+    # a field of two timeslices (the smallest lattice the library has), and only the part of that field that holds
+    # timeslice 0 goes on the wire: in the device layout (include/qcd.h) its even sites are the checkerboard indices
+    # [0, Vs/2) and its odd ones [Vs, Vs + Vs/2), i.e. two runs of 32-site chunks, and a face without time-like links
+    # (mask 0x7) needs the first 27 of the 36 units per site.  Per face that is about Vs x 72 (54) reals instead of
+    # the 2 Vs x 72 of the whole two-timeslice field.
+    def _face_chunks(self):
+        if getattr(self, "_chunks", None) is None:
+            h = self.Vs // 2
+            idx = sorted(set(range(0, (h + 31) // 32)) | set(range(self.Vs // 32, (self.Vs + h - 1) // 32 + 1)))
+            self._chunks = torch.tensor(idx, dtype=torch.int64, device="cuda")
+        return self._chunks
+
+    @staticmethod
+    def _face_units(mask):
+        return 27 if mask == MASK_SPATIAL else 36
+
     def face(self, te, mask, stream=None):
+        """the links `mask` of stored timeslice te as a message: [chunks of timeslice 0][units][32][2], contiguous"""
         buf = self.face_lat.new_matrix_field(self.dtype)
         self.qcd.qcd_copy_timeslices(self.lat, self.U, te, self.face_lat, buf, 0, 1, 72, mask, stream)
-        return buf
+        return buf[self._face_chunks(), : self._face_units(mask)].contiguous()
 
-    def put_face(self, buf, te, mask, stream=None):
+    def put_face(self, msg, te, mask, stream=None):
+        buf = self.face_lat.new_matrix_field(self.dtype)
+        buf[self._face_chunks(), : self._face_units(mask)] = msg
         self.qcd.qcd_copy_timeslices(self.face_lat, buf, 0, self.lat, self.U, te, 1, 72, mask, stream)
+
+    def gather(self, which):
+        """the interior timeslices of this slab as a canonical host array [t_count * Vs, 4, 3, 3]"""
+        a = self.qcd.field_to_host(self.lat, self.U if which == "U" else self.P)
+        return a.reshape(self.n + 2, self.Vs, 4, 3, 3)[1: self.n + 1].reshape(-1, 4, 3, 3)
 
     def observables(self):
         """per interior timeslice: plaquette average and K = sum |P_ij|^2 (device tensors of length t_count)"""
@@ -251,9 +295,8 @@ class SlabSet:
         import numpy as np
         out = []
         for s in self.slabs:
-            a = self.qcd.field_to_host(s.lat, s.U if which == "U" else s.P)
-            out.append(a.reshape(s.n + 2, s.Vs, 4, 3, 3)[1: s.n + 1])
-        return np.concatenate(out).reshape(-1, 4, 3, 3)
+            out.append(s.gather(which))
+        return np.concatenate(out)
 
     def global_observables(self):
         per_t, kt = zip(*(s.observables() for s in self.slabs))

@@ -3,6 +3,10 @@ into 2 and 4 slabs in one process, halos travel through qcd_copy_timeslices (wha
 do), and the gathered result must equal the undecomposed lattice — bit for bit for the generator, and for the
 trajectory because every site runs the same arithmetic in the same order whatever tile it falls in — and the
 oracle within the usual tolerance.  PAPER.md:24 (multi-GPU support), PAPER.md:121 (overlap, work in progress)."""
+import os
+import socket
+import time
+
 import numpy as np
 import pytest
 
@@ -183,3 +187,111 @@ def test_copy_timeslices_arguments(qcd):
     got, src = qcd.field_to_host(a, Uc).reshape(10, 512, 4, 3, 3), qcd.field_to_host(a, Ua).reshape(10, 512, 4, 3, 3)
     assert np.array_equal(got[5, :, 0], src[2, :, 0]) and np.array_equal(got[5, :, 2], src[2, :, 2])
     assert np.all(got[5, :, 1] == 0) and np.all(got[5, :, 3] == 0) and np.all(got[4] == 0)
+
+
+# ---- DistSlab: one slab per PROCESS, faces through torch.distributed (the class a multi-GPU job runs) ----------
+
+def _full_lattice_leapfrog(qcd, dims, prec, beta, eps, n, seed):
+    full = qcd.Lattice(dims)
+    dt = tdtype(prec)
+    fU, fP = full.new_matrix_field(dt), full.new_matrix_field(dt)
+    qcd.qcd_hot_start(full, fU, seed, 0.5)
+    qcd.qcd_mom_refresh(full, fP, seed)
+    qcd.qcd_leapfrog(full, fU, fP, beta, eps, n)
+    return host(qcd, full, fU), host(qcd, full, fP)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 16), (4, 6, 2, 8), (2, 2, 2, 4)])
+def test_dist_slab_alone_equals_the_whole_lattice(qcd, dims, prec):
+    """world = 1: the slab's halos are its own boundary timeslices, sent to itself as compact face messages (only the
+    chunks of one timeslice, three links for the face that goes down); bit-identical to qcd_leapfrog"""
+    import torch
+    from paper_1212_0785_b200 import slabs
+    beta, eps, n, seed = 5.8, 0.05, 3, 0x1212078500000002
+    wU, wP = _full_lattice_leapfrog(qcd, dims, prec, beta, eps, n, seed)
+    ds = slabs.DistSlab(qcd, dims, slabs.SlabComm(0, 1), tdtype(prec))
+    ds.start(seed, 0.5)
+    ds.leapfrog(beta, eps, n)
+    torch.cuda.synchronize()
+    assert np.array_equal(ds.gather("U"), wU) and np.array_equal(ds.gather("P"), wP)
+    # a face message holds one timeslice, not the two-timeslice staging field
+    Vs = dims[0] * dims[1] * dims[2]
+    up, down = ds.face(ds.n, slabs.MASK_ALL), ds.face(1, slabs.MASK_SPATIAL)
+    assert up.shape[1:] == (36, 32, 2) and down.shape[1:] == (27, 32, 2)
+    assert up.shape[0] <= (Vs // 2 + 31) // 32 * 2 + 1 and up.is_contiguous() and down.is_contiguous()
+    # and the observables are the whole lattice's
+    full = qcd.Lattice(dims)
+    ws = full.new_workspace()
+    avg = torch.zeros(1, dtype=torch.float64, device="cuda")
+    per_t = torch.zeros(dims[3], dtype=torch.float64, device="cuda")
+    qcd.qcd_plaquette(full, qcd.field_to_device(full, wU, tdtype(prec)), avg, per_t, ws)
+    plaq, K, plaq_t = ds.global_observables(beta)
+    # (the two parities of a timeslice are summed in the slab's local order: equal up to rounding, not bit for bit)
+    assert np.abs(plaq_t.cpu().numpy() - per_t.cpu().numpy()).max() < TOL[prec] and abs(plaq - avg.item()) < TOL[prec]
+
+
+def _dist_slab_worker(rank, world, port, out, dims, prec, beta, eps, n, seed):
+    """one rank of a DistSlab job: every rank uses cuda:0 (the box has one GPU); faces and reductions travel over gloo
+    through host memory.  The ranks' kernels never wait on one another: each rank's host blocks in the exchange."""
+    import datetime
+
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world, timeout=datetime.timedelta(seconds=90))
+    torch.cuda.set_device(0)
+    from paper_1212_0785_b200 import binding as qcd
+    from paper_1212_0785_b200 import slabs
+    ds = slabs.DistSlab(qcd, dims, slabs.SlabComm(rank, world, dist), tdtype(prec))
+    ds.start(seed, 0.5)
+    ds.leapfrog(beta, eps, n)
+    plaq, K, plaq_t = ds.global_observables(beta)
+    torch.cuda.synchronize()
+    np.savez(f"{out}.{rank}.npz", U=ds.gather("U"), P=ds.gather("P"), plaq=plaq, K=K, plaq_t=plaq_t.cpu().numpy(),
+             t_begin=ds.t_begin, t_count=ds.n)
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("dims,world,prec", [((8, 8, 8, 16), 2, "f64"), ((4, 6, 2, 12), 3, "f64"), ((8, 8, 8, 16), 2, "f32")])
+def test_dist_slab_processes_equal_the_whole_lattice(qcd, orc_omp, tmp_path, dims, world, prec):
+    """the decomposition as a multi-GPU job runs it — one process per slab, halo faces exchanged between processes
+     — here with all processes on the one GPU and gloo as the transport: the gathered trajectory is
+    bit-identical to the undecomposed run and within tolerance of the oracle, and every rank holds the same global
+    observables"""
+    import torch
+    import torch.multiprocessing as mp
+    beta, eps, n, seed = 5.8, 0.05, 3, 0x1212078500000002
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "ds")
+    ctx = mp.start_processes(_dist_slab_worker, args=(world, port, out, dims, prec, beta, eps, n, seed), nprocs=world,
+                             join=False, start_method="spawn")
+    deadline = time.time() + 240.0
+    try:
+        while not ctx.join(timeout=5.0):
+            assert time.time() < deadline, "DistSlab ranks did not finish"
+    finally:
+        for p in ctx.processes:  # only the processes this test started
+            if p.is_alive():
+                p.kill()
+    res = [np.load(f"{out}.{r}.npz") for r in range(world)]
+    assert [int(x["t_begin"]) for x in res] == sorted(int(x["t_begin"]) for x in res)
+    gU, gP = np.concatenate([x["U"] for x in res]), np.concatenate([x["P"] for x in res])
+    wU, wP = _full_lattice_leapfrog(qcd, dims, prec, beta, eps, n, seed)
+    assert np.array_equal(gU, wU) and np.array_equal(gP, wP)
+    full = qcd.Lattice(dims)
+    dt = tdtype(prec)
+    fU, fP = full.new_matrix_field(dt), full.new_matrix_field(dt)
+    qcd.qcd_hot_start(full, fU, seed, 0.5)
+    qcd.qcd_mom_refresh(full, fP, seed)
+    rU, rP = orc_omp.leapfrog(dims, beta, eps, n, host(qcd, full, fU), host(qcd, full, fP))
+    assert rel(gU, rU) < TOL[prec] and rel(gP, rP) < TOL[prec]
+    rplaq, rper_t = orc_omp.plaquette(dims, rU)
+    rK = orc_omp.sum(dims, O.SUM_NORM2, rP.view(np.float64).reshape(full.V, 72))[0]
+    for x in res:
+        assert float(x["plaq"]) == float(res[0]["plaq"]) and float(x["K"]) == float(res[0]["K"])
+        assert np.array_equal(x["plaq_t"], res[0]["plaq_t"]) and x["plaq_t"].shape == (dims[3],)
+        assert abs(float(x["plaq"]) - rplaq) < TOL[prec] and abs(float(x["K"]) - rK) < TOL[prec] * rK
+        assert np.abs(x["plaq_t"] - rper_t).max() < TOL[prec]
