@@ -61,25 +61,6 @@ __device__ __forceinline__ void load_link(M3<T> &m, const pair_t<T> *__restrict_
     }
 }
 
-// SU(3) links only: load rows 0 and 1 (6 of the 9 entries) and rebuild row 2 = conj(r0 x r1), the relation
-// reunit() (O9) imposes.  Two thirds of the bytes through L1/L2 for 36 extra FMAs per link.
-template <typename T>
-__device__ __forceinline__ void load_link_su3(M3<T> &m, const pair_t<T> *__restrict__ f, int V, int mu, int cb) {
-    const pair_t<T> *p = f + unit_index(36, mu * 9, cb);
-#pragma unroll
-    for (int e = 0; e < 6; e++) {
-        pair_t<T> v = __ldg(p + e * CHUNK);
-        m.re[e] = v.x;
-        m.im[e] = v.y;
-    }
-#pragma unroll
-    for (int j = 0; j < 3; j++) {
-        const int a = (j + 1) % 3, b = (j + 2) % 3;
-        m.re[6 + j] = m.re[a] * m.re[3 + b] - m.im[a] * m.im[3 + b] - (m.re[b] * m.re[3 + a] - m.im[b] * m.im[3 + a]);
-        m.im[6 + j] = -(m.re[a] * m.im[3 + b] + m.im[a] * m.re[3 + b] - (m.re[b] * m.im[3 + a] + m.im[b] * m.re[3 + a]));
-    }
-}
-
 // streaming variants (ld.global.cs / st.global.cs): for data touched once per kernel (the momenta in the
 // force kernel), so that it does not displace the neighbour links other threads of the block reuse from L1
 template <typename T>
