@@ -13,6 +13,8 @@ config 4, 32^3x64 fp64, sigma=0.2, beta=6.0, eps=0.02, seeded synthetic hot star
 
 N > 1 (torchrun): the path is run as N independent replicas (one lattice per GPU, different seeds,
 no data-path collective); value = total site-updates/s, scaling "weak".
+--decompose instead cuts ONE lattice into N slabs of timeslices, one per rank, with a halo exchange per step
+(strong scaling; its own JSON object).
 
 --impl reference times the CPU oracle (oracle/, as it stands, serial) on a bounded sample of the
 same workload; rank 0 only.
@@ -432,6 +434,68 @@ def run_slabs(args, cfg):
                       "closing half kick"}}), flush=True)
 
 
+def run_decompose(args, cfg):
+    """--decompose: ONE lattice cut into --gpus slabs of timeslices, one per rank (paper_1212_0785_b200/slabs.py
+    DistSlab): the leapfrog step as a multi-GPU job runs it — link update (exp + reunit),
+    one halo exchange (two face messages per rank through torch.distributed: NCCL batch_isend_irecv for N > 1, the
+    rank's own boundary for N = 1), force + momentum update.  Strong scaling: the lattice is fixed, value = V x steps /
+    the slowest rank's device time.  One JSON object; the headline line stays the replica run."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1212_0785_b200 import binding as qcd
+    from paper_1212_0785_b200 import slabs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = local % torch.cuda.device_count() if args.backend == "gloo" else local
+    torch.cuda.set_device(local)
+    if world > 1 and args.backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    elif world > 1:  # gloo: several ranks may share a GPU (faces staged through the host); a functional check only
+        dist.init_process_group("gloo")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dtype = torch.float64 if args.dtype == "f64" else torch.float32
+    dims, beta, eps = cfg["dims"], cfg["beta"], cfg["eps"]
+    V = dims[0] * dims[1] * dims[2] * dims[3]
+    ds = slabs.DistSlab(qcd, dims, slabs.SlabComm(rank, world, dist if world > 1 else None), dtype)
+    ds.start(SEED_BASE + 4, cfg["sigma"])  # the generator is keyed on the global site: every rank uses the same seed
+    ds.exchange()
+    ds.leapfrog(beta, eps, max(args.warmup, 3))
+    K = args.steps
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    ds.leapfrog(beta, eps, K)
+    e1.record()
+    barrier()
+    value, ms = aggregate(e0.elapsed_time(e1), V / world, K, world, "cuda")
+    plaq, kin, _ = ds.global_observables(beta)  # collective: every rank takes part
+    face = ds.face(ds.n, slabs.MASK_ALL).numel() + ds.face(1, slabs.MASK_SPATIAL).numel()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": f"{cfg['name']} {args.dtype} leapfrog, the lattice cut into {world} slab(s) of "
+                                   f"{ds.n} timeslices, one per rank; per step: link update (exp + reunit), one halo "
+                                   "exchange, force + momentum update; the timed region also holds the opening half kick",
+                       "mode": "decompose", "transport": "own boundary (one rank)" if world == 1 else "NCCL batch_isend_irecv" if args.backend == "nccl"
+                                    else "gloo through host memory (functional check, not a measurement)",
+                       "sent_bytes_per_rank_per_step": face * (8 if args.dtype == "f64" else 4)},
+            "plaquette": plaq, "kinetic_energy": kin}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_per_kernel(args, cfg):
     """each kernel alone on ALL / EVEN / ODD with an L2 flush between timed launches (config 3's U + P is about the
     size of L2); one JSON line with a list of rows"""
@@ -528,6 +592,12 @@ def main():
     ap.add_argument("--slabs", type=int, default=0,
                     help="instead of the MD-step line: the step on the lattice cut into this many slabs of timeslices in one "
                          "process (in-kernel halo push), against the undecomposed step")
+    ap.add_argument("--decompose", action="store_true",
+                    help="instead of the MD-step line: ONE lattice cut into --gpus slabs of timeslices, one per rank, halo "
+                         "faces exchanged through torch.distributed (strong scaling; the default N > 1 run is replicas)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="--decompose only: gloo lets several ranks share one GPU (faces staged through host memory) to "
+                         "check the N > 1 code path on a one-GPU box; its timings are not measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-kernel", action="store_true",
                     help="instead of the MD-step line: every kernel alone on ALL/EVEN/ODD with an L2 flush between "
@@ -542,6 +612,8 @@ def main():
         run_reference(args, cfg)
     elif args.peaks:
         run_peaks(args)
+    elif args.decompose:
+        run_decompose(args, cfg)
     elif args.slabs > 0:
         run_slabs(args, cfg)
     elif args.per_kernel:

@@ -909,7 +909,7 @@ def test_config_trajectory_full_size_against_oracle(qcd, orc_omp, cfg, prec, n):
     """BASELINE configs 4 and 5 at full size ("sustained 20-step leapfrog trajectory with per-step
     reunitarization and reductions ... reports dH"): qcd_trajectory against the OpenMP build of the oracle,
     step by step — plaquette, per-timeslice plaquette and K of every step, dH (R15: against |H|), final links and
-    momenta at sampled sites.  Config 5 fp64 runs all 20 steps; the other two rows are shortened to 4 and 2 steps
+    momenta at sampled sites, and at EVERY site for config 4.  Config 5 fp64 runs all 20 steps; the other two rows are shortened to 4 and 2 steps
     to keep the suite's time down (the oracle needs about 9 s per 48^3x96 step on 16 host cores)."""
     import torch
     c = inputs.CONFIGS[cfg]
@@ -941,6 +941,9 @@ def test_config_trajectory_full_size_against_oracle(qcd, orc_omp, cfg, prec, n):
         return (g[..., 0] + 1j * g[..., 1]).T.reshape(len(sites), 4, 3, 3)
 
     assert rel(gather(dU), rU[sites]) < TOL[prec] and rel(gather(dP), rP[sites]) < TOL[prec]
+    if cfg == 4:  # every link of every site as well (a 1.2 GB unpack per field; config 5 would need 6 GB per copy)
+        assert rel(host(qcd, lat, dU), rU) < TOL[prec]
+        assert rel(host(qcd, lat, dP), rP) < TOL[prec]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])

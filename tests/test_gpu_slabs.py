@@ -3,8 +3,11 @@ into 2 and 4 slabs in one process, halos travel through qcd_copy_timeslices (wha
 do), and the gathered result must equal the undecomposed lattice — bit for bit for the generator, and for the
 trajectory because every site runs the same arithmetic in the same order whatever tile it falls in — and the
 oracle within the usual tolerance.  PAPER.md:24 (multi-GPU support), PAPER.md:121 (overlap, work in progress)."""
+import json
 import os
 import socket
+import subprocess
+import sys
 import time
 
 import numpy as np
@@ -295,3 +298,25 @@ def test_dist_slab_processes_equal_the_whole_lattice(qcd, orc_omp, tmp_path, dim
         assert np.array_equal(x["plaq_t"], res[0]["plaq_t"]) and x["plaq_t"].shape == (dims[3],)
         assert abs(float(x["plaq"]) - rplaq) < TOL[prec] and abs(float(x["K"]) - rK) < TOL[prec] * rK
         assert np.abs(x["plaq_t"] - rper_t).max() < TOL[prec]
+
+
+@pytest.mark.parametrize("world", [1, 2])
+def test_bench_decompose_mode_runs(world):
+    """bench.py --decompose (one lattice cut into one slab per rank, DistSlab) prints one strong-scaling JSON object;
+    world = 2: two ranks share the one GPU over gloo — a check of the N > 1 code path, not a measurement"""
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    tail = [os.path.join(root, "bench.py"), "--gpus", str(world), "--decompose", "--config", "3", "--steps", "2"]
+    cmd = [sys.executable] + tail if world == 1 else \
+        [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world), "--master-addr",
+         "127.0.0.1", "--master-port", str(port)] + tail + ["--backend", "gloo"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=root)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1  # rank 0 only
+    d = json.loads(lines[0])
+    assert d["scaling"] == "strong" and d["n_gpus"] == world and d["config"]["mode"] == "decompose"
+    assert d["value"] > 0 and 0.0 < d["plaquette"] < 1.0 and d["kinetic_energy"] > 0
+    assert d["config"]["sent_bytes_per_rank_per_step"] == 16 ** 3 * (72 + 54) * 8  # one timeslice up, three links down
